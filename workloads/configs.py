@@ -1,0 +1,223 @@
+"""Input generators for BASELINE.json configs 1-5 (recipes: SURVEY.md 8(d)).
+
+No method arithmetic lives here: only initial conditions and parameter dicts.
+"""
+from dataclasses import dataclass, field
+from typing import Dict, Optional, Tuple
+
+import numpy as np
+import torch
+
+from .analytic import layered_channel_closed_form
+
+
+def _closed_form_T(*a, **k):
+    u, v, T, U = layered_channel_closed_form(*a, **k)
+    if not np.all(np.isfinite(T)):
+        T = np.full_like(T, 0.5 * (k["T_h"] + k["T_c"]))
+    return u, v, T, U
+
+
+@dataclass
+class Workload:
+    name: str
+    nx: int
+    ny: int
+    nz: int
+    params: dict                      # keys as in tcp_params (see include/tcp.h)
+    phi: torch.Tensor                 # [nz][ny][nx] float64
+    u: Optional[torch.Tensor] = None  # [3][nz][ny][nx] or None (=> 0)
+    T: Optional[torch.Tensor] = None  # [nz][ny][nx] or None (=> T_ref)
+    wall_T: Dict[Tuple[int, int], torch.Tensor] = field(default_factory=dict)  # (axis, face) -> plane
+    steps: int = 100
+    notes: str = ""
+
+    @property
+    def cells(self) -> int:
+        return self.nx * self.ny * self.nz
+
+
+def _grid(nx, ny, nz, device="cpu"):
+    z = torch.arange(nz, dtype=torch.float64, device=device).view(nz, 1, 1)
+    y = torch.arange(ny, dtype=torch.float64, device=device).view(1, ny, 1)
+    x = torch.arange(nx, dtype=torch.float64, device=device).view(1, 1, nx)
+    return x, y, z
+
+
+def _droplet_profile(r, R, xi):
+    """phi = 1 inside, 0 outside, tanh profile of width xi (eq. 35 form)."""
+    return 0.5 * (1.0 - torch.tanh(2.0 * (r - R) / xi))
+
+
+# --------------------------------------------------------------------------------------------
+# config 1: static droplet, fully periodic cube
+
+def static_droplet(n=32, R=8.0, thermal="lb_d3q7", nz=None):
+    """BASELINE.json configs[0].  nz=1 gives the quasi-2-D (cylinder) variant used by the
+    Laplace pin."""
+    nz = n if nz is None else nz
+    x, y, z = _grid(n, n, nz)
+    c = (n - 1) / 2.0
+    r2 = (x - c) ** 2 + (y - c) ** 2
+    if nz > 1:
+        r2 = r2 + (z - (nz - 1) / 2.0) ** 2
+    r = torch.sqrt(r2).expand(nz, n, n).contiguous()
+    params = dict(thermal=thermal, bc=("periodic",) * 3,
+                  rho_H=10.0, rho_L=1.0, tau_H=0.8, tau_L=0.8, xi=4.0, M=0.02,
+                  sigma_ref=1e-3, sigma_T=0.0, T_ref=0.0,
+                  kappa_H=0.2, kappa_L=0.2, cp_H=1.0, cp_L=1.0)
+    return Workload("static_droplet", n, n, nz, params, _droplet_profile(r, R, 4.0), steps=200)
+
+
+# --------------------------------------------------------------------------------------------
+# config 2: layered thermocapillary channel
+
+def layered_channel(nx=256, ny=128, nz=1, thermal="lb_d3q7", kappa_upper=0.2, rho_upper=1.0,
+                    cp_upper=1.0):
+    """BASELINE.json configs[1].  x, z periodic; no-slip walls at y = -1/2 and y = ny - 1/2.
+    Lower half phi = 0 (fluid B, next to the heated wall), upper half phi = 1 (fluid A).
+    T0 is the closed-form steady temperature (App. A)."""
+    T_h, T_c, T_0 = 20.0, 10.0, 4.0
+    xi, nu, kappa_B = 4.0, 0.2, 0.2
+    a = b = ny / 2.0
+    x, y, z = _grid(nx, ny, nz)
+    yi = (y - (ny / 2.0 - 0.5))             # distance from the interface (between the middle cells)
+    phi = (0.5 * (1.0 + torch.tanh(2.0 * yi / xi))).expand(nz, ny, nx).contiguous()
+    k_r = kappa_upper / kappa_B
+    mu_r = rho_upper * 1.0                  # same kinematic viscosity in both layers
+    sigma_T = -5e-4
+    xn = np.arange(nx, dtype=np.float64)[None, :]
+    yn = (np.arange(ny, dtype=np.float64) - (ny / 2.0 - 0.5))[:, None]
+    with np.errstate(all="ignore"):   # nx = 1 (1-D test set-ups) overflows the x-dependent part; T0 is then replaced below
+        _, _, Tcf, _ = _closed_form_T(xn, yn, a=a, b=b, L=float(nx), T_h=T_h, T_c=T_c,
+                                               T_0=T_0, k_r=k_r, mu_r=mu_r, mu_B=nu * 1.0,
+                                               sigma_T=sigma_T)
+    T = torch.from_numpy(np.broadcast_to(Tcf, (nz, ny, nx)).copy())
+    params = dict(thermal=thermal, bc=("periodic", "walls", "periodic"),
+                  rho_H=rho_upper, rho_L=1.0, tau_H=3.0 * nu, tau_L=3.0 * nu, xi=xi, M=0.05,
+                  sigma_ref=2.5e-2, sigma_T=sigma_T, T_ref=T_c,
+                  kappa_H=kappa_upper, kappa_L=kappa_B, cp_H=cp_upper, cp_L=1.0,
+                  wall_T=((0.0, 0.0), (T_h, T_c), (0.0, 0.0)))
+    xs = torch.arange(nx, dtype=torch.float64)
+    Tw_bottom = (T_h + T_0 * torch.cos(2.0 * np.pi * xs / nx)).view(1, nx).expand(nz, nx).contiguous()
+    wl = Workload("layered_channel", nx, ny, nz, params, phi, T=T,
+                  wall_T={(1, 0): Tw_bottom}, steps=20000)
+    wl.notes = "closed form: a=b=ny/2, L=nx, mu_B=nu*rho_L"
+    return wl
+
+
+# --------------------------------------------------------------------------------------------
+# config 3: droplet migrating in a linear temperature gradient
+
+def droplet_in_gradient(nx=128, ny=128, nz=256, thermal="lb_d3q19", R=16.0, zc=64.0, grad_T=0.01):
+    """BASELINE.json configs[2].  Walls at z (T = 0 at the bottom, grad_T * nz at the top: 2.55
+    is the value 0.01 * 255 of the config rounded to the half-cell wall position), periodic x, y."""
+    xi = 5.0
+    x, y, z = _grid(nx, ny, nz)
+    r = torch.sqrt((x - (nx - 1) / 2.0) ** 2 + (y - (ny - 1) / 2.0) ** 2 + (z - zc) ** 2)
+    phi = _droplet_profile(r, R, xi)
+    T_top = grad_T * nz if nz != 256 else 2.55
+    T = ((z + 0.5) / nz * T_top).expand(nz, ny, nx).contiguous()
+    params = dict(thermal=thermal, bc=("periodic", "periodic", "walls"),
+                  rho_H=1.0, rho_L=1.0, tau_H=0.6, tau_L=0.6, xi=xi, M=0.05,
+                  sigma_ref=2.5e-2, sigma_T=-5e-4, T_ref=0.0,
+                  kappa_H=0.2, kappa_L=0.2, cp_H=1.0, cp_L=1.0,
+                  wall_T=((0.0, 0.0), (0.0, 0.0), (0.0, T_top)))
+    return Workload("droplet_in_gradient", nx, ny, nz, params, phi, T=T, steps=5000)
+
+
+# --------------------------------------------------------------------------------------------
+# config 4: thermal-tweezer droplet capture
+
+BENCH_FLUID = dict(rho_H=10.0, rho_L=1.0, tau_H=0.5, tau_L=0.05, xi=5.0, M=0.02,
+                   sigma_ref=5e-3, sigma_T=-2e-4, T_ref=0.0,
+                   kappa_H=0.2, kappa_L=0.2, cp_H=1.0, cp_L=1.0)
+
+
+def thermal_tweezer(nx=256, ny=256, nz=128, thermal="rk2", R=20.0, offset=60.0, A=10.0, s=20.0):
+    """BASELINE.json configs[3].  Bottom wall (z face 0) carries T_ref + A exp(-r^2/(2 s^2)) about
+    the axis; top wall at T_ref; droplet centred `offset` cells off-axis in x at height R + xi,
+    initial velocity 1e-3 toward the axis inside the droplet."""
+    xi = BENCH_FLUID["xi"]
+    x, y, z = _grid(nx, ny, nz)
+    ax, ay = (nx - 1) / 2.0, (ny - 1) / 2.0
+    zc = R + xi
+    r = torch.sqrt((x - (ax + offset)) ** 2 + (y - ay) ** 2 + (z - zc) ** 2)
+    phi = _droplet_profile(r, R, xi)
+    u = torch.zeros(3, nz, ny, nx, dtype=torch.float64)
+    u[0] = -1e-3 * phi
+    xs = torch.arange(nx, dtype=torch.float64).view(1, nx)
+    ys = torch.arange(ny, dtype=torch.float64).view(ny, 1)
+    Tw = A * torch.exp(-((xs - ax) ** 2 + (ys - ay) ** 2) / (2.0 * s * s))
+    params = dict(BENCH_FLUID, thermal=thermal, bc=("periodic", "periodic", "walls"))
+    return Workload("thermal_tweezer", nx, ny, nz, params, phi, u=u, T=None,
+                    wall_T={(2, 0): Tw.contiguous()}, steps=10000)
+
+
+# --------------------------------------------------------------------------------------------
+# config 5: performance boxes
+
+def perf_box(n, thermal="lb_d3q7", seed=None, device="cpu", nz=None, ny=None, volume_fraction=0.10,
+             r_min=8.0, r_max=24.0):
+    """BASELINE.json configs[4]: fully periodic box with seeded, randomly placed non-overlapping
+    droplets (radius uniform in [8,24], ~10 % volume fraction) and a smoothed random temperature
+    (uniform in [0,1], then 10 Jacobi passes: T <- mean of the 6 face neighbours)."""
+    nx = n
+    ny = n if ny is None else ny
+    nz = n if nz is None else nz
+    seed = 20240103 + n if seed is None else seed
+    rng = np.random.default_rng(seed)
+    xi = BENCH_FLUID["xi"]
+    ext = np.array([nx, ny, nz], dtype=np.float64)
+    r_max = min(r_max, 0.25 * min(nx, ny, nz))
+    r_min = min(r_min, r_max)
+    target = volume_fraction * nx * ny * nz
+    centres, radii, vol, tries = [], [], 0.0, 0
+    while vol < target and tries < 200000:
+        tries += 1
+        R = rng.uniform(r_min, r_max)
+        c = rng.uniform(0.0, 1.0, 3) * ext
+        ok = True
+        for c2, R2 in zip(centres, radii):
+            d = np.abs(c - c2)
+            d = np.minimum(d, ext - d)          # minimum image
+            if np.sqrt((d ** 2).sum()) < R + R2 + xi:
+                ok = False
+                break
+        if ok:
+            centres.append(c); radii.append(R); vol += 4.0 / 3.0 * np.pi * R ** 3
+    phi = torch.zeros(nz, ny, nx, dtype=torch.float64, device=device)
+    for c, R in zip(centres, radii):
+        # paint each droplet on its own (periodically wrapped) bounding box only
+        h = int(np.ceil(R + 4 * xi))
+        idx = []
+        dist2 = 0.0
+        for a, (cc, nn) in enumerate(zip(c, (nx, ny, nz))):
+            i0 = int(np.floor(cc)) - h
+            ii = torch.arange(i0, i0 + 2 * h + 2, device=device)
+            if ii.numel() > nn:
+                ii = torch.arange(nn, device=device)
+            d = torch.abs((ii % nn).to(torch.float64) - cc)
+            d = torch.minimum(d, nn - d)
+            idx.append(ii % nn)
+            shape = [1, 1, 1]
+            shape[2 - a] = -1
+            dist2 = dist2 + (d ** 2).view(shape)
+        prof = _droplet_profile(torch.sqrt(dist2), R, xi)
+        iz, iy, ix = idx[2].view(-1, 1, 1), idx[1].view(1, -1, 1), idx[0].view(1, 1, -1)
+        phi[iz, iy, ix] = torch.clamp(phi[iz, iy, ix] + prof, 0.0, 1.0)
+    gen = torch.Generator(device="cpu").manual_seed(seed)
+    if device == "cpu" or nx * ny * nz <= (1 << 24):
+        T = torch.rand(nz, ny, nx, dtype=torch.float64, generator=gen).to(device)
+    else:
+        # big boxes: draw on the device (only the CUDA path runs them; the sampled-parity test reads
+        # sub-boxes back from these very tensors, so the oracle still sees identical inputs)
+        dgen = torch.Generator(device=device).manual_seed(seed)
+        T = torch.rand(nz, ny, nx, dtype=torch.float64, generator=dgen, device=device)
+    for _ in range(10):
+        T = (torch.roll(T, 1, 0) + torch.roll(T, -1, 0) + torch.roll(T, 1, 1) + torch.roll(T, -1, 1)
+             + torch.roll(T, 1, 2) + torch.roll(T, -1, 2)) / 6.0
+    params = dict(BENCH_FLUID, thermal=thermal, bc=("periodic",) * 3)
+    wl = Workload(f"perf_box_{nx}x{ny}x{nz}", nx, ny, nz, params, phi, T=T, steps=100)
+    wl.notes = f"{len(radii)} droplets, seed {seed}"
+    return wl

@@ -1,0 +1,283 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPS of the full coupled thermocapillary step (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--size 400] [--thermal lb_d3q7]
+                    [--precision f64] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (phase-field LB, hydrodynamic LB, temperature update)
+over the box.  Default workload: the 400^3 fp64 D3Q27/D3Q27/D3Q7 periodic box of BASELINE.json
+configs[4] (seeded random droplets + smoothed random temperature; synthetic, the paper's workloads
+are synthetic set-ups too).  Prints ONE JSON line (rank 0).
+
+N > 1 (torchrun): the path has no data-path collective here -- every rank advances its own box
+("replicas", weak scaling); the time is the max over ranks, the value the sum of cells.
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the
+same workload on the host cores; it is a deliberately slow program, reported as a baseline only.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+import workloads as W
+
+METRIC = "MLUPS of full coupled step on 1 B200; % of HBM roofline (bytes/cell)"
+QT = {"lb_d3q7": 7, "lb_d3q15": 15, "lb_d3q19": 19, "lb_d3q27": 27, "rk2": 0, "rk4": 0}
+
+
+def fused_kernel_values_per_cell(thermal):
+    """Algorithmic values moved per cell by the dominant kernel: h, g read +
+    written (54 + 54), f read + written (2 Q_T), phi read + written (2), T read (+ written on the LB
+    path), u read + written (6)."""
+    q = QT[thermal]
+    return 54 + 54 + 2 * q + 2 + (2 if q else 1) + 6
+
+
+def step_values_per_cell(thermal):
+    v = fused_kernel_values_per_cell(thermal)
+    if thermal == "rk2":      # stage: read Y, phi, u(3), Tn; write out
+        v += 2 * 7
+    if thermal == "rk4":      # + accumulator read/write on stages 1-4
+        v += 7 + 9 + 9 + 7
+    return v
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def recorded_traffic(key):
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        return json.load(open(path)).get(key)
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_throughput(thermal, n=40, warm=1, steps=6):
+    """The oracle, as it stands, on a bounded sample of the workload (n^3 box, same recipe)."""
+    from oracle import tcpo
+    wl = W.perf_box(n, thermal=thermal, r_min=4.0, r_max=8.0)
+    o = tcpo.Oracle(n, n, n, wl.params)
+    o.init_fields(wl.phi.numpy(), None, wl.T.numpy())
+    o.step(warm)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    o.close()
+    return n ** 3 * steps / dt / 1e6, dt / steps, tcpo.num_threads(), f"{n}^3 periodic perf box (same recipe, fluid and thermal variant), {warm} warm-up + {steps} timed steps"
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = args.ref_size
+    vals = []
+    per_step = []
+    for _ in range(1):
+        v, ms, cores, sample = oracle_throughput(args.thermal, n=n, warm=min(args.warmup, 2), steps=max(1, min(args.steps, 8)))
+        vals.append(v); per_step.append(ms)
+    value = vals[0]
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_step[0] * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"perf_box {args.size}^3 periodic, thermal {args.thermal} (oracle timed on a {n}^3 sample)"},
+            "cpu_baseline": {"value": value, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import paper_2401_03041_b200 as tcp
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    n, thermal, prec = args.size, args.thermal, args.precision
+    es = 8 if prec == "f64" else 4
+    tdt = torch.float64 if prec == "f64" else torch.float32
+    wl = W.perf_box(n, thermal=thermal, device="cuda", seed=20240103 + n + rank)
+    N = wl.cells
+    params = dict(wl.params, precision=prec)
+    sim = tcp.Simulation(n, n, n, params)
+    phi_d, T_d = wl.phi.to(tdt).contiguous(), wl.T.to(tdt).contiguous()
+    sim.init_fields(phi_d, None, T_d)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps --------------------------
+    sim.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sim.launches
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(sim.stream)
+    sim.step(args.steps)
+    ev1.record(sim.stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    kernel_ms = sim.last_step_ms()            # events recorded by the library around its own launches
+    launches = sim.launches - l0
+    clocks = sampler.stop() if rank == 0 else None
+    t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = world * N * args.steps / (ms_max * 1e-3) / 1e6
+    phi_chk = sim.read_fields_device()[0]
+    finite = bool(torch.isfinite(phi_chk).all().item())
+    sum_drift = abs(float(phi_chk.double().sum().item()) - float(phi_d.double().sum().item())) / float(phi_d.double().sum().item())
+    del phi_chk
+
+    # ---- end to end through the C ABI with HOST buffers ---------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hp = torch.empty((n, n, n), dtype=tdt, pin_memory=True); hp.copy_(phi_d)
+        hT = torch.empty((n, n, n), dtype=tdt, pin_memory=True); hT.copy_(T_d)
+        hu = torch.zeros((3, n, n, n), dtype=tdt, pin_memory=True)
+        o_phi = torch.empty((n, n, n), dtype=tdt, pin_memory=True); o_T = torch.empty_like(o_phi); o_p = torch.empty_like(o_phi)
+        o_u = torch.empty((3, n, n, n), dtype=tdt, pin_memory=True)
+        barrier()
+        t0 = time.perf_counter()
+        tcp.tcp_init_fields(sim._h, hp, hu, hT)            # H2D of phi, u, T + equilibrium init
+        tcp.tcp_step(sim._h, args.steps)
+        tcp.tcp_read_fields(sim._h, o_phi, o_u, o_p, o_T)  # pressure kernel + D2H of phi, u, p, T (synchronises)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+        if dist:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * N * args.steps / float(t.item()) / 1e6, "unit": "MLUPS",
+               "h2d_bytes_per_step": 5 * N * es / args.steps, "d2h_bytes_per_step": 6 * N * es / args.steps,
+               "note": f"tcp_init_fields(host) + tcp_step({args.steps}) + tcp_read_fields(host), pinned host buffers"}
+        del hp, hT, hu, o_phi, o_T, o_p, o_u
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = hbm_peak()
+    fused_bytes = fused_kernel_values_per_cell(thermal) * es * N
+    step_bytes = step_values_per_cell(thermal) * es * N
+    if QT[thermal]:
+        k_ms = kernel_ms / args.steps                      # one fused kernel per step
+        achieved = fused_bytes / (k_ms * 1e-3) / 1e9
+        kname = "fused_step_kernel"
+    else:
+        k_ms = kernel_ms / args.steps
+        achieved = step_bytes / (k_ms * 1e-3) / 1e9        # whole step (fused kernel + RK stages)
+        kname = "fused_step_kernel + rk_stage_kernel (whole step)"
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": recorded_traffic(f"{thermal}_{prec}_{n}"), "kernel": kname, "peak_source": peak_src,
+                "algorithmic_bytes_per_cell": (fused_bytes if QT[thermal] else step_bytes) / N,
+                "kernel_ms": k_ms}
+    cpu = None
+    if not args.no_cpu:
+        v, _, cores, sample = oracle_throughput(thermal)
+        cpu = {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample}
+    line = {"metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": prec, "data": "synthetic",
+            "config": {"workload": f"perf_box {n}^3 periodic (BASELINE configs[4]), hydro D3Q27 CM, phase D3Q27, thermal {thermal}",
+                       "cells_per_gpu": N, "parallelism": "replicas" if world > 1 else "single GPU",
+                       "l2": f"working set {step_bytes / 1e9:.1f} GB per step >> 126 MB L2, no flush needed",
+                       "notes": wl.notes},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "checks": {"finite": finite, "sum_phi_rel_drift": sum_drift}}
+    print(json.dumps(line), flush=True)
+    if dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--size", type=int, default=400)
+    ap.add_argument("--thermal", default="lb_d3q7", choices=sorted(QT))
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-size", type=int, default=40)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                   # timing rule: W >= 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

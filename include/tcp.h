@@ -1,0 +1,116 @@
+/*
+ * tcp.h -- C ABI of the B200-native thermocapillary central-moment phase-field lattice Boltzmann
+ * step (arxiv 2401.03041; citations are PAPER.md:<line> of the reference text).
+ *
+ * One `tcp_sim` holds the state of one simulation on one GPU: the post-collision populations
+ * h~ (D3Q27, phase field, eq. 10), g~ (D3Q27, hydrodynamics, eq. 16),
+ * f~ (D3Q7/15/19/27, temperature, eq. 27; absent on the Runge-Kutta paths) and the
+ * fields phi, u, T.  `tcp_step` advances it by Algorithm 1 / Algorithm 2.
+ *
+ * Conventions
+ *   - cell index = x + nx*(y + ny*z), x fastest; every cell is fluid; a WALLS axis has no-slip,
+ *     fixed-temperature walls half a cell outside its first and last cell.
+ *   - arrays are in the simulation's precision (double for TCP_F64, float for TCP_F32);
+ *     vector fields are 3 planes [3][nz][ny][nx].
+ *   - array arguments may be HOST or DEVICE pointers (resolved with cudaMemcpyDefault); the
+ *     caller owns them, the library copies.  Wall planes: axis 0 -> [nz][ny], 1 -> [nz][nx],
+ *     2 -> [ny][nx].
+ *   - every function returns TCP_OK (0) or a negative TCP_E* code, never throws or aborts;
+ *     `tcp_last_error()` gives a thread-local message for the last failure on this thread.
+ *   - there is no CPU fallback: without a CUDA device every call that needs one fails with
+ *     TCP_ECUDA.
+ */
+#ifndef TCP_H
+#define TCP_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tcp_sim tcp_sim; /* opaque; owned by the library; freed by tcp_destroy */
+
+enum { TCP_OK = 0, TCP_EINVAL = -1, TCP_ENOMEM = -2, TCP_ECUDA = -3, TCP_EUNSUPPORTED = -4, TCP_ESTATE = -5 };
+enum { TCP_F64 = 0, TCP_F32 = 1 };
+enum { TCP_THERMAL_LB_D3Q7 = 0, TCP_THERMAL_LB_D3Q15, TCP_THERMAL_LB_D3Q19, TCP_THERMAL_LB_D3Q27,
+       TCP_THERMAL_RK2, TCP_THERMAL_RK4 };
+enum { TCP_BC_PERIODIC = 0, TCP_BC_WALLS = 1 };
+enum { TCP_STREAM_TWO_GRID = 0, TCP_STREAM_AA = 1 }; /* AA: not built yet -> TCP_EUNSUPPORTED */
+
+/* The paper's problem statement (sections 2.1-2.3).  Fill `struct_size = sizeof(tcp_params)`. */
+typedef struct tcp_params {
+    unsigned struct_size;
+    int precision;                     /* TCP_F64 | TCP_F32 */
+    int thermal;                       /* TCP_THERMAL_*: eqs. 27-29 (LB) or eqs. 25-26 with eq. 4 (RK) */
+    int streaming;                     /* TCP_STREAM_* */
+    int bc[3];                         /* TCP_BC_* for x, y, z */
+    double rho_H, rho_L;               /* eq. 14 */
+    double tau_H, tau_L;               /* eq. 22; nu = tau c_s^2, rate 1/(tau+1/2) */
+    double xi, M;                      /* interface width, mobility: eqs. 3, 11, 15 */
+    double sigma_ref, sigma_T, T_ref;  /* eq. 9 */
+    double kappa_H, kappa_L, cp_H, cp_L; /* eqs. 23-24; rho and c_p enter only the RK paths (eq. 4) */
+    double gravity[3];                 /* eq. 7 */
+    double wall_T[3][2];               /* constant wall temperature per axis / face (eqs. 30-31) */
+    double s_bulk, s_high;             /* central-moment rates of the trace of the 2nd-order moments and of
+                                          all moments of order >= 3 (hydrodynamic lattice); default 1, 1.
+                                          s_high != 1 is TCP_EUNSUPPORTED unless high_rate_equals_shear */
+    int high_rate_equals_shear;        /* 1: every rate = the physical one = plain BGK + Guo */
+    double eps_normal;                 /* n = grad phi / sqrt(|grad phi|^2 + eps); default 1e-32 */
+} tcp_params;
+
+/* Bytes of device memory one simulation needs (populations, fields, wall planes).
+ * Errors: TCP_EINVAL (bad extents / parameters), TCP_EUNSUPPORTED. */
+int tcp_workspace_bytes(int nx, int ny, int nz, const tcp_params *p, size_t *bytes);
+
+/* Create a simulation; the library allocates the workspace (cudaMalloc) and a stream.
+ * Validation: n >= 1 (>= 2 on WALLS axes), tau > -1/2, M, xi, rho, kappa, cp > 0.
+ * Errors: TCP_EINVAL, TCP_EUNSUPPORTED, TCP_ENOMEM, TCP_ECUDA. */
+int tcp_create(int nx, int ny, int nz, const tcp_params *p, tcp_sim **out);
+
+/* Same, on caller-owned device memory (>= tcp_workspace_bytes, 256-byte aligned) and on the
+ * caller's CUDA stream (a cudaStream_t passed as void*; NULL = default stream).  The memory and
+ * the stream must outlive the simulation. */
+int tcp_create_in(int nx, int ny, int nz, const tcp_params *p, void *dev_workspace, size_t bytes,
+                  void *cuda_stream, tcp_sim **out);
+
+/* Set phi, u, T and initialise all populations to their equilibria:
+ * h~ = h_eq(phi, u) (eq. 12), g~ = g_eq(p* = 0, u) (eq. 18), f~ = f_eq(T, u).
+ * u == NULL -> 0; T == NULL -> T_ref.  Errors: TCP_EINVAL (phi NULL), TCP_ECUDA. */
+int tcp_init_fields(tcp_sim *s, const void *phi, const void *u, const void *T);
+
+/* Per-wall-cell Dirichlet temperature (eq. 30); Tw == NULL restores the constant wall_T. */
+int tcp_set_wall_temperature(tcp_sim *s, int axis, int face, const void *Tw);
+
+/* Volumetric heat source q_T [nz][ny][nx] of eqs. 4 / 27 (e.g. eq. 37); NULL (default) = none. */
+int tcp_set_heat_source(tcp_sim *s, const void *q);
+
+/* Advance nsteps time steps: per step, the phase-field update (eqs. 10-15), the hydrodynamic
+ * update (eqs. 16-22 with the forces of eqs. 7-9) and the temperature update (eqs. 27-29, or
+ * eq. 4 by eq. 26 / eq. 25).  Asynchronous on the simulation's stream.
+ * Errors: TCP_ESTATE (fields not initialised), TCP_EINVAL (nsteps < 0), TCP_ECUDA. */
+int tcp_step(tcp_sim *s, int nsteps);
+
+/* Copy out phi, u, p = c_s^2 rho(phi) sum_i g~_i, T; any pointer may be NULL.
+ * Synchronises the stream. */
+int tcp_read_fields(tcp_sim *s, void *phi, void *u, void *p, void *T);
+
+/* Wait for all work of this simulation.  Errors: TCP_ECUDA (incl. asynchronous kernel faults). */
+int tcp_synchronize(tcp_sim *s);
+
+/* Number of kernels this simulation has launched so far (bench.py's gpu_launches). */
+long long tcp_launch_count(const tcp_sim *s);
+
+/* Time the last tcp_step call spent on the device, in milliseconds, measured with CUDA events
+ * recorded on the simulation's stream around the kernels of that call (synchronises).
+ * Errors: TCP_ESTATE if tcp_step has not been called. */
+int tcp_last_step_ms(tcp_sim *s, float *ms);
+
+int tcp_destroy(tcp_sim *s);
+
+const char *tcp_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TCP_H */

@@ -1,0 +1,415 @@
+// Host side of the C ABI declared in include/tcp.h: workspace layout, launches, copies.
+// There is no CPU path: every entry point that computes launches CUDA kernels.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/tcp.h"
+#include "tcp_step.cuh"
+
+namespace {
+
+thread_local char g_err[512];
+
+int fail(int code, const char* fmt, const char* detail = "") {
+    std::snprintf(g_err, sizeof g_err, fmt, detail);
+    return code;
+}
+int cuda_fail(cudaError_t e, const char* where) {
+    std::snprintf(g_err, sizeof g_err, "%s: %s", where, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? TCP_ENOMEM : TCP_ECUDA;
+}
+#define CK(call)                                                  \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);       \
+    } while (0)
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+int thermal_q(int thermal) {
+    switch (thermal) {
+    case TCP_THERMAL_LB_D3Q7: return 7;
+    case TCP_THERMAL_LB_D3Q15: return 15;
+    case TCP_THERMAL_LB_D3Q19: return 19;
+    case TCP_THERMAL_LB_D3Q27: return 27;
+    default: return 0;
+    }
+}
+
+// byte offsets of every array inside the workspace
+struct Layout {
+    size_t h[2], g[2], f[2], phi[2], T[2], u, rk[3], wallT[3][2], q, total;
+};
+
+int validate(int nx, int ny, int nz, const tcp_params* p) {
+    if (!p) return fail(TCP_EINVAL, "params is NULL");
+    if (p->struct_size != sizeof(tcp_params)) return fail(TCP_EINVAL, "tcp_params.struct_size != sizeof(tcp_params)");
+    if (nx < 1 || ny < 1 || nz < 1) return fail(TCP_EINVAL, "extents must be >= 1");
+    if ((double)nx * ny * nz >= 2147483647.0) return fail(TCP_EINVAL, "nx*ny*nz must be < 2^31");
+    const int n[3] = {nx, ny, nz};
+    for (int a = 0; a < 3; ++a) {
+        if (p->bc[a] != TCP_BC_PERIODIC && p->bc[a] != TCP_BC_WALLS) return fail(TCP_EINVAL, "bc must be TCP_BC_PERIODIC or TCP_BC_WALLS");
+        if (p->bc[a] == TCP_BC_WALLS && n[a] < 2) return fail(TCP_EINVAL, "a WALLS axis needs at least 2 cells");
+    }
+    if (p->precision != TCP_F64 && p->precision != TCP_F32) return fail(TCP_EINVAL, "bad precision");
+    if (p->thermal < TCP_THERMAL_LB_D3Q7 || p->thermal > TCP_THERMAL_RK4) return fail(TCP_EINVAL, "bad thermal variant");
+    if (p->streaming != TCP_STREAM_TWO_GRID && p->streaming != TCP_STREAM_AA) return fail(TCP_EINVAL, "bad streaming pattern");
+    if (!(p->tau_H > -0.5) || !(p->tau_L > -0.5)) return fail(TCP_EINVAL, "tau must be > -1/2");
+    if (!(p->M > 0) || !(p->xi > 0)) return fail(TCP_EINVAL, "M and xi must be > 0");
+    if (!(p->rho_H > 0) || !(p->rho_L > 0)) return fail(TCP_EINVAL, "rho must be > 0");
+    if (!(p->kappa_H > 0) || !(p->kappa_L > 0) || !(p->cp_H > 0) || !(p->cp_L > 0)) return fail(TCP_EINVAL, "kappa and cp must be > 0");
+    if (!(p->eps_normal >= 0)) return fail(TCP_EINVAL, "eps_normal must be >= 0");
+    if (p->streaming == TCP_STREAM_AA) return fail(TCP_EUNSUPPORTED, "AA in-place streaming is not built yet");
+    if (!p->high_rate_equals_shear && p->s_high != 1.0)
+        return fail(TCP_EUNSUPPORTED, "s_high != 1 needs the general central-moment transform (not built yet)");
+    return TCP_OK;
+}
+
+Layout make_layout(int nx, int ny, int nz, const tcp_params* p) {
+    Layout L;
+    std::memset(&L, 0, sizeof L);
+    const size_t es = p->precision == TCP_F64 ? 8 : 4;
+    const size_t N = (size_t)nx * ny * nz;
+    const int QT = thermal_q(p->thermal);
+    size_t off = 0;
+    auto take = [&](size_t count) { size_t o = off; off = align_up(off + count * es); return o; };
+    for (int b = 0; b < 2; ++b) L.h[b] = take(27 * N);
+    for (int b = 0; b < 2; ++b) L.g[b] = take(27 * N);
+    for (int b = 0; b < 2; ++b) L.f[b] = QT ? take((size_t)QT * N) : 0;
+    for (int b = 0; b < 2; ++b) L.phi[b] = take(N);
+    for (int b = 0; b < 2; ++b) L.T[b] = take(N);
+    L.u = take(3 * N);
+    const int nrk = p->thermal == TCP_THERMAL_RK2 ? 1 : (p->thermal == TCP_THERMAL_RK4 ? 3 : 0);
+    for (int k = 0; k < nrk; ++k) L.rk[k] = take(N);
+    const size_t plane[3] = {(size_t)ny * nz, (size_t)nx * nz, (size_t)nx * ny};
+    for (int a = 0; a < 3; ++a)
+        for (int fc = 0; fc < 2; ++fc) L.wallT[a][fc] = take(plane[a]);
+    L.q = take(N);
+    L.total = off;
+    return L;
+}
+
+}  // namespace
+
+struct tcp_sim {
+    int nx, ny, nz;
+    size_t N;
+    tcp_params P;
+    Layout L;
+    char* base;
+    bool owns_memory, owns_stream;
+    cudaStream_t stream;
+    int cur;                 // index of the buffers holding time level n
+    bool initialised, has_q, walls, stepped;
+    long long launches;
+    cudaEvent_t ev0, ev1;
+};
+
+namespace {
+
+template <typename real> real* ptr(const tcp_sim* s, size_t off) { return reinterpret_cast<real*>(s->base + off); }
+
+template <typename real>
+tcp::StepArgs<real> make_args(const tcp_sim* s) {
+    tcp::StepArgs<real> A;
+    std::memset(&A, 0, sizeof A);
+    const tcp_params& P = s->P;
+    const int c = s->cur, o = 1 - s->cur;
+    A.nx = s->nx; A.ny = s->ny; A.nz = s->nz; A.ncell = (int)s->N;
+    for (int a = 0; a < 3; ++a) A.wall[a] = P.bc[a] == TCP_BC_WALLS;
+    A.h_in = ptr<real>(s, s->L.h[c]); A.h_out = ptr<real>(s, s->L.h[o]);
+    A.g_in = ptr<real>(s, s->L.g[c]); A.g_out = ptr<real>(s, s->L.g[o]);
+    A.f_in = ptr<real>(s, s->L.f[c]); A.f_out = ptr<real>(s, s->L.f[o]);
+    A.phi_in = ptr<real>(s, s->L.phi[c]); A.phi_out = ptr<real>(s, s->L.phi[o]);
+    A.T_in = ptr<real>(s, s->L.T[c]); A.T_out = ptr<real>(s, s->L.T[o]);
+    A.u = ptr<real>(s, s->L.u);
+    A.q_src = s->has_q ? ptr<real>(s, s->L.q) : nullptr;
+    for (int a = 0; a < 3; ++a)
+        for (int fc = 0; fc < 2; ++fc) A.wallT[a][fc] = ptr<real>(s, s->L.wallT[a][fc]);
+    A.rho_L = (real)P.rho_L; A.drho = (real)(P.rho_H - P.rho_L);
+    A.tau_L = (real)P.tau_L; A.dtau = (real)(P.tau_H - P.tau_L);
+    A.xi = (real)P.xi; A.w_phi = (real)(1.0 / (0.5 + 3.0 * P.M));
+    A.sigma_ref = (real)P.sigma_ref; A.sigma_T = (real)P.sigma_T; A.T_ref = (real)P.T_ref;
+    A.kappa_L = (real)P.kappa_L; A.dkappa = (real)(P.kappa_H - P.kappa_L);
+    A.cp_L = (real)P.cp_L; A.dcp = (real)(P.cp_H - P.cp_L);
+    for (int a = 0; a < 3; ++a) A.grav[a] = (real)P.gravity[a];
+    A.s_bulk = (real)P.s_bulk;
+    // S8: eps keeps n = grad phi / |grad phi| finite where grad phi vanishes.  In fp32 a gradient
+    // below ~1e-6 is round-off of phi ~ 1, and a round-off-directed sharpening flux makes phi = 0 / 1
+    // unstable to noise (measured: 1e-4 error after 100 steps next to a wall), so eps is floored there.
+    A.eps = (real)(sizeof(real) == 4 ? std::fmax(P.eps_normal, 1e-12) : P.eps_normal);
+    return A;
+}
+
+unsigned grid_for(size_t n) { return (unsigned)((n + tcp::kBlock - 1) / tcp::kBlock); }
+
+template <typename real, bool WALLS, bool BGK>
+void launch_fused(const tcp_sim* s, const tcp::StepArgs<real>& A) {
+    const unsigned grid = grid_for(s->N);
+    switch (thermal_q(s->P.thermal)) {
+    case 7: tcp::fused_step_kernel<real, 7, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 15: tcp::fused_step_kernel<real, 15, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 19: tcp::fused_step_kernel<real, 19, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 27: tcp::fused_step_kernel<real, 27, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    default: tcp::fused_step_kernel<real, 0, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    }
+}
+
+template <typename real>
+void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
+    const unsigned grid = grid_for(s->N);
+    if (s->walls) tcp::rk_stage_kernel<real, true><<<grid, tcp::kBlock, 0, s->stream>>>(R);
+    else tcp::rk_stage_kernel<real, false><<<grid, tcp::kBlock, 0, s->stream>>>(R);
+}
+
+// one time step: Algorithm 1 (thermal LB, one fused kernel) or Algorithm 2 (fused phase+hydro
+// kernel, then the Runge-Kutta stages)
+template <typename real>
+int step_once(tcp_sim* s) {
+    tcp::StepArgs<real> A = make_args<real>(s);
+    const bool bgk = s->P.high_rate_equals_shear != 0;
+    if (s->walls) { if (bgk) launch_fused<real, true, true>(s, A); else launch_fused<real, true, false>(s, A); }
+    else          { if (bgk) launch_fused<real, false, true>(s, A); else launch_fused<real, false, false>(s, A); }
+    s->launches++;
+    const int th = s->P.thermal;
+    if (th == TCP_THERMAL_RK2 || th == TCP_THERMAL_RK4) {
+        tcp::RkArgs<real> R;
+        std::memset(&R, 0, sizeof R);
+        R.S = A;
+        R.S.phi_in = A.phi_out;              // phi^{n+1}; u already holds u^{n+1}
+        real* Tn = ptr<real>(s, s->L.T[s->cur]);
+        real* Tnew = ptr<real>(s, s->L.T[1 - s->cur]);
+        real* Ya = ptr<real>(s, s->L.rk[0]);
+        R.Tn = Tn;
+        if (th == TCP_THERMAL_RK2) {         // eq. 26 (G6)
+            R.Y = Tn; R.out = Ya; R.c_out = (real)0.5; R.mode = 0;
+            launch_rk_stage<real>(s, R);
+            R.Y = Ya; R.out = Tnew; R.c_out = (real)1.0; R.mode = 0;
+            launch_rk_stage<real>(s, R);
+            s->launches += 2;
+        } else {                             // eq. 25
+            real* Yb = ptr<real>(s, s->L.rk[1]);
+            real* acc = ptr<real>(s, s->L.rk[2]);
+            R.acc_in = acc; R.acc_out = acc;
+            R.Y = Tn; R.out = Ya; R.c_out = (real)0.5; R.c_acc = (real)(1.0 / 6.0); R.mode = 1;
+            launch_rk_stage<real>(s, R);
+            R.Y = Ya; R.out = Yb; R.c_out = (real)0.5; R.c_acc = (real)(1.0 / 3.0); R.mode = 2;
+            launch_rk_stage<real>(s, R);
+            R.Y = Yb; R.out = Ya; R.c_out = (real)1.0; R.c_acc = (real)(1.0 / 3.0); R.mode = 2;
+            launch_rk_stage<real>(s, R);
+            R.Y = Ya; R.out = Tnew; R.c_acc = (real)(1.0 / 6.0); R.mode = 3;
+            launch_rk_stage<real>(s, R);
+            s->launches += 4;
+        }
+    }
+    s->cur = 1 - s->cur;
+    return TCP_OK;
+}
+
+template <typename real>
+int init_fields_t(tcp_sim* s, const void* phi, const void* u, const void* T) {
+    const size_t N = s->N, es = sizeof(real);
+    s->cur = 0;
+    CK(cudaMemcpyAsync(ptr<real>(s, s->L.phi[0]), phi, N * es, cudaMemcpyDefault, s->stream));
+    if (u) CK(cudaMemcpyAsync(ptr<real>(s, s->L.u), u, 3 * N * es, cudaMemcpyDefault, s->stream));
+    else CK(cudaMemsetAsync(ptr<real>(s, s->L.u), 0, 3 * N * es, s->stream));
+    if (T) CK(cudaMemcpyAsync(ptr<real>(s, s->L.T[0]), T, N * es, cudaMemcpyDefault, s->stream));
+    else {
+        tcp::fill_kernel<real><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(ptr<real>(s, s->L.T[0]), (long long)N, (real)s->P.T_ref);
+        s->launches++;
+    }
+    tcp::StepArgs<real> A = make_args<real>(s);
+    A.h_out = ptr<real>(s, s->L.h[0]); A.g_out = ptr<real>(s, s->L.g[0]); A.f_out = ptr<real>(s, s->L.f[0]);
+    const unsigned grid = grid_for(N);
+    switch (thermal_q(s->P.thermal)) {
+    case 7: tcp::init_kernel<real, 7><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 15: tcp::init_kernel<real, 15><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 19: tcp::init_kernel<real, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 27: tcp::init_kernel<real, 27><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    default: tcp::init_kernel<real, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    }
+    s->launches++;
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(s->stream));   // the caller may free its arrays when we return
+    s->initialised = true;
+    return TCP_OK;
+}
+
+template <typename real>
+int fill_wall(tcp_sim* s, int axis, int face, const void* Tw) {
+    const size_t plane[3] = {(size_t)s->ny * s->nz, (size_t)s->nx * s->nz, (size_t)s->nx * s->ny};
+    real* dst = ptr<real>(s, s->L.wallT[axis][face]);
+    if (Tw) CK(cudaMemcpyAsync(dst, Tw, plane[axis] * sizeof(real), cudaMemcpyDefault, s->stream));
+    else {
+        tcp::fill_kernel<real><<<(unsigned)((plane[axis] + 255) / 256), 256, 0, s->stream>>>(dst, (long long)plane[axis],
+                                                                                        (real)s->P.wall_T[axis][face]);
+        s->launches++;
+        CK(cudaGetLastError());
+    }
+    CK(cudaStreamSynchronize(s->stream));
+    return TCP_OK;
+}
+
+template <typename real>
+int read_fields_t(tcp_sim* s, void* phi, void* u, void* p, void* T) {
+    const size_t N = s->N, es = sizeof(real);
+    if (phi) CK(cudaMemcpyAsync(phi, ptr<real>(s, s->L.phi[s->cur]), N * es, cudaMemcpyDefault, s->stream));
+    if (u) CK(cudaMemcpyAsync(u, ptr<real>(s, s->L.u), 3 * N * es, cudaMemcpyDefault, s->stream));
+    if (T) CK(cudaMemcpyAsync(T, ptr<real>(s, s->L.T[s->cur]), N * es, cudaMemcpyDefault, s->stream));
+    if (p) {
+        real* scratch = ptr<real>(s, s->L.phi[1 - s->cur]);   // free between steps
+        tcp::pressure_kernel<real><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(ptr<real>(s, s->L.g[s->cur]), ptr<real>(s, s->L.phi[s->cur]),
+                                                                               scratch, (int)N, (real)s->P.rho_L,
+                                                                               (real)(s->P.rho_H - s->P.rho_L));
+        s->launches++;
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(p, scratch, N * es, cudaMemcpyDefault, s->stream));
+    }
+    CK(cudaStreamSynchronize(s->stream));
+    return TCP_OK;
+}
+
+int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, size_t bytes, void* stream, bool own, tcp_sim** out) {
+    if (!out) return fail(TCP_EINVAL, "out is NULL");
+    *out = nullptr;
+    int rc = validate(nx, ny, nz, p);
+    if (rc) return rc;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(TCP_ECUDA, "no CUDA device: this library has no CPU path");
+    }
+    tcp_sim* s = new (std::nothrow) tcp_sim();
+    if (!s) return fail(TCP_ENOMEM, "host allocation failed");
+    s->nx = nx; s->ny = ny; s->nz = nz; s->N = (size_t)nx * ny * nz; s->P = *p;
+    s->L = make_layout(nx, ny, nz, p);
+    s->walls = p->bc[0] == TCP_BC_WALLS || p->bc[1] == TCP_BC_WALLS || p->bc[2] == TCP_BC_WALLS;
+    s->owns_memory = own; s->owns_stream = own;
+    if (own) {
+        void* mem = nullptr;
+        e = cudaMalloc(&mem, s->L.total);
+        if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaMalloc(workspace)"); }
+        s->base = static_cast<char*>(mem);
+        e = cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { cudaFree(mem); delete s; return cuda_fail(e, "cudaStreamCreate"); }
+    } else {
+        if (!workspace) { delete s; return fail(TCP_EINVAL, "workspace is NULL"); }
+        if (bytes < s->L.total) { delete s; return fail(TCP_EINVAL, "workspace smaller than tcp_workspace_bytes"); }
+        if (reinterpret_cast<size_t>(workspace) % kAlign) { delete s; return fail(TCP_EINVAL, "workspace must be 256-byte aligned"); }
+        s->base = static_cast<char*>(workspace);
+        s->stream = static_cast<cudaStream_t>(stream);
+    }
+    if (cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess) {
+        tcp_destroy(s);
+        return fail(TCP_ECUDA, "cudaEventCreate failed");
+    }
+    for (int a = 0; a < 3; ++a)
+        for (int fc = 0; fc < 2; ++fc) {
+            rc = p->precision == TCP_F64 ? fill_wall<double>(s, a, fc, nullptr) : fill_wall<float>(s, a, fc, nullptr);
+            if (rc) { tcp_destroy(s); return rc; }
+        }
+    *out = s;
+    return TCP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tcp_last_error(void) { return g_err; }
+
+int tcp_workspace_bytes(int nx, int ny, int nz, const tcp_params* p, size_t* bytes) {
+    if (!bytes) return fail(TCP_EINVAL, "bytes is NULL");
+    int rc = validate(nx, ny, nz, p);
+    if (rc) return rc;
+    *bytes = make_layout(nx, ny, nz, p).total;
+    return TCP_OK;
+}
+
+int tcp_create(int nx, int ny, int nz, const tcp_params* p, tcp_sim** out) {
+    return create_common(nx, ny, nz, p, nullptr, 0, nullptr, true, out);
+}
+
+int tcp_create_in(int nx, int ny, int nz, const tcp_params* p, void* dev_workspace, size_t bytes, void* cuda_stream, tcp_sim** out) {
+    return create_common(nx, ny, nz, p, dev_workspace, bytes, cuda_stream, false, out);
+}
+
+int tcp_destroy(tcp_sim* s) {
+    if (!s) return TCP_OK;
+    cudaStreamSynchronize(s->stream);
+    if (s->ev0) cudaEventDestroy(s->ev0);
+    if (s->ev1) cudaEventDestroy(s->ev1);
+    if (s->owns_stream && s->stream) cudaStreamDestroy(s->stream);
+    if (s->owns_memory && s->base) cudaFree(s->base);
+    delete s;
+    return TCP_OK;
+}
+
+int tcp_init_fields(tcp_sim* s, const void* phi, const void* u, const void* T) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (!phi) return fail(TCP_EINVAL, "phi is required");
+    return s->P.precision == TCP_F64 ? init_fields_t<double>(s, phi, u, T) : init_fields_t<float>(s, phi, u, T);
+}
+
+int tcp_set_wall_temperature(tcp_sim* s, int axis, int face, const void* Tw) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (axis < 0 || axis > 2 || face < 0 || face > 1) return fail(TCP_EINVAL, "axis must be 0..2 and face 0..1");
+    return s->P.precision == TCP_F64 ? fill_wall<double>(s, axis, face, Tw) : fill_wall<float>(s, axis, face, Tw);
+}
+
+int tcp_set_heat_source(tcp_sim* s, const void* q) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    s->has_q = q != nullptr;
+    if (q) {
+        const size_t es = s->P.precision == TCP_F64 ? 8 : 4;
+        CK(cudaMemcpyAsync(s->base + s->L.q, q, s->N * es, cudaMemcpyDefault, s->stream));
+        CK(cudaStreamSynchronize(s->stream));
+    }
+    return TCP_OK;
+}
+
+int tcp_step(tcp_sim* s, int nsteps) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
+    if (nsteps < 0) return fail(TCP_EINVAL, "nsteps must be >= 0");
+    CK(cudaEventRecord(s->ev0, s->stream));
+    for (int n = 0; n < nsteps; ++n) {
+        int rc = s->P.precision == TCP_F64 ? step_once<double>(s) : step_once<float>(s);
+        if (rc) return rc;
+    }
+    CK(cudaEventRecord(s->ev1, s->stream));
+    CK(cudaGetLastError());
+    s->stepped = true;
+    return TCP_OK;
+}
+
+int tcp_read_fields(tcp_sim* s, void* phi, void* u, void* p, void* T) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
+    return s->P.precision == TCP_F64 ? read_fields_t<double>(s, phi, u, p, T) : read_fields_t<float>(s, phi, u, p, T);
+}
+
+int tcp_synchronize(tcp_sim* s) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    CK(cudaStreamSynchronize(s->stream));
+    CK(cudaGetLastError());
+    return TCP_OK;
+}
+
+long long tcp_launch_count(const tcp_sim* s) { return s ? s->launches : 0; }
+
+int tcp_last_step_ms(tcp_sim* s, float* ms) {
+    if (!s || !ms) return fail(TCP_EINVAL, "NULL argument");
+    if (!s->stepped) return fail(TCP_ESTATE, "tcp_step has not been called");
+    CK(cudaEventSynchronize(s->ev1));
+    CK(cudaEventElapsedTime(ms, s->ev0, s->ev1));
+    return TCP_OK;
+}
+
+}  // extern "C"

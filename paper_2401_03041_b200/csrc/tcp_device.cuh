@@ -1,0 +1,297 @@
+// Device-side building blocks of the coupled step: neighbourhoods and boundary rules, the
+// isotropic finite differences, moments, and the closed-form central-moment collisions.
+//
+// Citations are PAPER.md:<line>.  Readings of the paper (S*/G*/A*) are listed in DESIGN.md.
+// This file shares nothing with oracle/ (the CPU oracle builds dense moment matrices; here the
+// same operator is evaluated in closed form).
+#pragma once
+#include "tcp_lattice.cuh"
+
+namespace tcp {
+
+template <typename real>
+struct StepArgs {
+    int nx, ny, nz;
+    int ncell;                       // nx*ny*nz < 2^31
+    int wall[3];                     // 1 = WALLS on that axis
+    const real* h_in;  real* h_out;  // [27][N]
+    const real* g_in;  real* g_out;  // [27][N]
+    const real* f_in;  real* f_out;  // [QT][N] (thermal LB only)
+    const real* phi_in; real* phi_out;
+    const real* T_in;  real* T_out;
+    real* u;                         // [3][N], updated in place (only read locally)
+    const real* q_src;               // heat source or nullptr
+    const real* wallT[3][2];         // wall-temperature planes
+    real rho_L, drho, tau_L, dtau;   // eqs. 14, 22
+    real xi, w_phi;                  // eq. 15; rate 1/(1/2 + 3M) (eq. 11, reading G3)
+    real sigma_ref, sigma_T, T_ref;  // eq. 9
+    real kappa_L, dkappa, cp_L, dcp; // eqs. 23-24 (reading G5)
+    real grav[3];                    // eq. 7
+    real s_bulk, eps;
+};
+
+// ---------------------------------------------------------------------------------------------
+// neighbourhood of one cell: element offsets to the 26 neighbours with periodic wrap, or, on a
+// WALLS axis, clamped to the mirror cell (reading S9: walls half a cell outside the end cells)
+
+template <bool WALLS>
+struct Nbh {
+    int idx;
+    int dx[3], dy[3], dz[3];         // offsets for c = -1, 0, +1
+    bool lo[3], hi[3];               // WALLS: the cell touches the low / high wall of axis a
+    int X[3], Y[3], Z[3];            // WALLS: coordinates of the wrapped / mirrored neighbours
+    int nx, ny;
+
+    template <typename real>
+    __device__ __forceinline__ void init(const StepArgs<real>& A, int cell) {
+        idx = cell;
+        nx = A.nx; ny = A.ny;
+        const int x = cell % A.nx;
+        const int t = cell / A.nx;
+        const int y = t % A.ny;
+        const int z = t / A.ny;
+        const int sy = A.nx, sz = A.nx * A.ny;
+        const bool wx = WALLS && A.wall[0], wy = WALLS && A.wall[1], wz = WALLS && A.wall[2];
+        dx[1] = dy[1] = dz[1] = 0;
+        dx[0] = x > 0 ? -1 : (wx ? 0 : A.nx - 1);
+        dx[2] = x < A.nx - 1 ? 1 : (wx ? 0 : -(A.nx - 1));
+        dy[0] = y > 0 ? -sy : (wy ? 0 : (A.ny - 1) * sy);
+        dy[2] = y < A.ny - 1 ? sy : (wy ? 0 : -(A.ny - 1) * sy);
+        dz[0] = z > 0 ? -sz : (wz ? 0 : (A.nz - 1) * sz);
+        dz[2] = z < A.nz - 1 ? sz : (wz ? 0 : -(A.nz - 1) * sz);
+        if (WALLS) {
+            lo[0] = wx && x == 0; hi[0] = wx && x == A.nx - 1;
+            lo[1] = wy && y == 0; hi[1] = wy && y == A.ny - 1;
+            lo[2] = wz && z == 0; hi[2] = wz && z == A.nz - 1;
+            X[1] = x; Y[1] = y; Z[1] = z;
+            X[0] = x + dx[0]; X[2] = x + dx[2];
+            Y[0] = y + dy[0] / sy; Y[2] = y + dy[2] / sy;
+            Z[0] = z + dz[0] / sz; Z[2] = z + dz[2] / sz;
+        }
+    }
+    __device__ __forceinline__ int at(int ox, int oy, int oz) const { return idx + dx[ox + 1] + dy[oy + 1] + dz[oz + 1]; }
+
+    // first wall axis (x, then y, then z) crossed when stepping by (ox,oy,oz); -1 if none
+    __device__ __forceinline__ int crossed(int ox, int oy, int oz, int& face) const {
+        if (!WALLS) return -1;
+        if (ox == -1 && lo[0]) { face = 0; return 0; }
+        if (ox == 1 && hi[0]) { face = 1; return 0; }
+        if (oy == -1 && lo[1]) { face = 0; return 1; }
+        if (oy == 1 && hi[1]) { face = 1; return 1; }
+        if (oz == -1 && lo[2]) { face = 0; return 2; }
+        if (oz == 1 && hi[2]) { face = 1; return 2; }
+        return -1;
+    }
+    // index into the tangential plane of wall `axis` at the neighbour (ox,oy,oz)
+    __device__ __forceinline__ int tangential(int axis, int ox, int oy, int oz) const {
+        const int xx = X[ox + 1], yy = Y[oy + 1], zz = Z[oz + 1];
+        return axis == 0 ? zz * ny + yy : (axis == 1 ? zz * nx + xx : yy * nx + xx);
+    }
+};
+
+template <typename real, bool WALLS>
+__device__ __forceinline__ real wall_temperature(const StepArgs<real>& A, const Nbh<WALLS>& nb, int axis, int face,
+                                                 int ox, int oy, int oz) {
+    return A.wallT[axis][face][nb.tangential(axis, ox, oy, oz)];
+}
+
+// ---------------------------------------------------------------------------------------------
+// isotropic finite differences with the D3Q27 weights (reading S3), evaluated as a tensor product:
+//   grad_x = D_x S_y S_z,  lap = 6 (S_x S_y S_z - 1),   S = [1/6, 2/3, 1/6],  D = [-1/2, 0, 1/2]
+// IS_TEMP: Dirichlet ghost 2 T_w - T(mirror); otherwise ghost = mirror cell (phi, neutral wetting).
+
+template <typename real, bool WALLS, bool IS_TEMP>
+__device__ __forceinline__ void stencil27(const StepArgs<real>& A, const Nbh<WALLS>& nb, const real* __restrict__ psi,
+                                          real& centre, real grad[3], real& lap) {
+    const real c16 = real(1.0 / 6.0), c23 = real(2.0 / 3.0), half = real(0.5);
+    real SS[3], DSy[3], SDx[3];
+#pragma unroll
+    for (int oz = -1; oz <= 1; ++oz) {
+        real sx[3], dxv[3];
+#pragma unroll
+        for (int oy = -1; oy <= 1; ++oy) {
+            real v[3];
+#pragma unroll
+            for (int ox = -1; ox <= 1; ++ox) {
+                real t = __ldg(psi + nb.at(ox, oy, oz));
+                if (WALLS && IS_TEMP) {
+                    int face = 0;
+                    const int ax = nb.crossed(ox, oy, oz, face);
+                    if (ax >= 0) t = real(2) * wall_temperature(A, nb, ax, face, ox, oy, oz) - t;
+                }
+                v[ox + 1] = t;
+            }
+            if (oy == 0 && oz == 0) centre = v[1];
+            sx[oy + 1] = (v[0] + v[2]) * c16 + v[1] * c23;
+            dxv[oy + 1] = (v[2] - v[0]) * half;
+        }
+        SS[oz + 1] = (sx[0] + sx[2]) * c16 + sx[1] * c23;
+        DSy[oz + 1] = (sx[2] - sx[0]) * half;
+        SDx[oz + 1] = (dxv[0] + dxv[2]) * c16 + dxv[1] * c23;
+    }
+    grad[0] = (SDx[0] + SDx[2]) * c16 + SDx[1] * c23;
+    grad[1] = (DSy[0] + DSy[2]) * c16 + DSy[1] * c23;
+    grad[2] = (SS[2] - SS[0]) * half;
+    lap = real(6) * (((SS[0] + SS[2]) * c16 + SS[1] * c23) - centre);
+}
+
+// ---------------------------------------------------------------------------------------------
+// pulls (two-grid): a_q(x) = a~_q(x - c_q); halfway bounce-back a~_opp(x) for h, g;
+// anti-bounce-back -f~_opp(x) + 2 w T_w for f (reading S9)
+
+template <typename real, bool WALLS>
+__device__ __forceinline__ void pull27(const StepArgs<real>& A, const Nbh<WALLS>& nb, const real* __restrict__ a, real out[27]) {
+    const long long N = A.ncell;
+#pragma unroll
+    for (int q = 0; q < 27; ++q) {
+        const int cx = cx27(q), cy = cy27(q), cz = cz27(q);
+        int face = 0;
+        if (WALLS && nb.crossed(-cx, -cy, -cz, face) >= 0)
+            out[q] = a[(26 - q) * N + nb.idx];
+        else
+            out[q] = a[q * N + nb.at(-cx, -cy, -cz)];
+    }
+}
+
+template <typename real, int Q, bool WALLS>
+__device__ __forceinline__ void pull_thermal(const StepArgs<real>& A, const Nbh<WALLS>& nb, const real* __restrict__ a, real out[Q]) {
+    const long long N = A.ncell;
+    static_for<0, Q>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(Q, k);
+        constexpr int cx = cx27(q), cy = cy27(q), cz = cz27(q);
+        int face = 0;
+        const int ax = nb.crossed(-cx, -cy, -cz, face);
+        if (WALLS && ax >= 0)
+            out[k] = real(2.0 * weight(Q, cls27(q))) * wall_temperature(A, nb, ax, face, -cx, -cy, -cz)
+                     - a[(Q - 1 - k) * N + nb.idx];
+        else
+            out[k] = a[k * N + nb.at(-cx, -cy, -cz)];
+    });
+}
+
+// ---------------------------------------------------------------------------------------------
+// raw moments of a D3Q27 population set up to order 2, by successive sums along x, y, z
+
+template <typename real>
+struct Mom2 {
+    real m0, mx, my, mz, mxx, myy, mzz, mxy, mxz, myz;
+};
+
+template <typename real, bool SECOND>
+__device__ __forceinline__ Mom2<real> moments27(const real a[27]) {
+    Mom2<real> M;
+    real t00[3], t01[3], t02[3], t10[3], t11[3], t20[3];
+#pragma unroll
+    for (int z = 0; z < 3; ++z) {
+        real s0[3], s1[3], s2[3];
+#pragma unroll
+        for (int y = 0; y < 3; ++y) {
+            const real m = a[9 * z + 3 * y], c = a[9 * z + 3 * y + 1], p = a[9 * z + 3 * y + 2];
+            s2[y] = p + m;
+            s0[y] = s2[y] + c;
+            s1[y] = p - m;
+        }
+        t00[z] = (s0[0] + s0[2]) + s0[1];
+        t01[z] = s0[2] - s0[0];
+        t10[z] = (s1[0] + s1[2]) + s1[1];
+        if (SECOND) {
+            t02[z] = s0[0] + s0[2];
+            t11[z] = s1[2] - s1[0];
+            t20[z] = (s2[0] + s2[2]) + s2[1];
+        }
+    }
+    M.m0 = (t00[0] + t00[2]) + t00[1];
+    M.mz = t00[2] - t00[0];
+    M.my = (t01[0] + t01[2]) + t01[1];
+    M.mx = (t10[0] + t10[2]) + t10[1];
+    if (SECOND) {
+        M.mzz = t00[0] + t00[2];
+        M.myz = t01[2] - t01[0];
+        M.myy = (t02[0] + t02[2]) + t02[1];
+        M.mxz = t10[2] - t10[0];
+        M.mxy = (t11[0] + t11[2]) + t11[1];
+        M.mxx = (t20[0] + t20[2]) + t20[1];
+    } else {
+        M.mxx = M.myy = M.mzz = M.mxy = M.mxz = M.myz = real(0);
+    }
+    return M;
+}
+
+// ---------------------------------------------------------------------------------------------
+// 1-D inverse central-moment columns on {-1, 0, +1}: r_k(c; u) is the population with k-th
+// central moment 1 and the other two 0
+template <typename real>
+struct R1D {
+    real r0[3], r1[3];   // index c+1; r2 = {1/2, -1, 1/2} is constant
+    __device__ __forceinline__ void set(real u) {
+        const real uu = u * u, hu = real(0.5) * u;
+        r0[0] = real(0.5) * uu - hu; r0[1] = real(1) - uu; r0[2] = real(0.5) * uu + hu;
+        r1[0] = u - real(0.5);       r1[1] = real(-2) * u; r1[2] = u + real(0.5);
+    }
+};
+
+// E_q = w_q [ A0 + 3 c.v + 4.5 (c.u)(c.b) ]  -- equilibrium (eq. 12 or eq. 18) plus half the Guo
+// force populations (ref. [20]), merged:
+//   scalar (h, f):  A0 = s - 1.5 u.b,  v = s u + a/2,  b = s u + a
+//   hydro  (g):     A0 = p* - 1.5 u.b, v = u + a/2,    b = u + a
+template <typename real>
+__device__ __forceinline__ void equilibrium_plus_half_force27(real A0, const real u[3], const real v[3], const real b[3], real out[27]) {
+#pragma unroll
+    for (int q = 0; q < 13; ++q) {
+        const int cx = cx27(q), cy = cy27(q), cz = cz27(q);
+        const real w = real(weight(27, cls27(q)));
+        const real cu = real(cx) * u[0] + real(cy) * u[1] + real(cz) * u[2];
+        const real cb = real(cx) * b[0] + real(cy) * b[1] + real(cz) * b[2];
+        const real cv = real(cx) * v[0] + real(cy) * v[1] + real(cz) * v[2];
+        const real sym = w * (A0 + real(4.5) * cu * cb);
+        const real asym = real(3) * w * cv;
+        out[q] = sym + asym;
+        out[26 - q] = sym - asym;
+    }
+    out[13] = real(weight(27, 0)) * A0;
+}
+
+// out_q += sum_alpha m_alpha R^alpha_q(u): populations whose first-order central moments are m and
+// whose other central moments vanish (tensor-product monomial basis of D3Q27, reading S2)
+template <typename real>
+__device__ __forceinline__ void add_first_order27(const real m[3], const R1D<real>& rx, const R1D<real>& ry, const R1D<real>& rz, real out[27]) {
+    real P[3][3], W[3][3];   // [cy][cx]
+#pragma unroll
+    for (int y = 0; y < 3; ++y)
+#pragma unroll
+        for (int x = 0; x < 3; ++x) {
+            P[y][x] = m[0] * rx.r1[x] * ry.r0[y] + m[1] * rx.r0[x] * ry.r1[y];
+            W[y][x] = m[2] * rx.r0[x] * ry.r0[y];
+        }
+#pragma unroll
+    for (int z = 0; z < 3; ++z)
+#pragma unroll
+        for (int y = 0; y < 3; ++y)
+#pragma unroll
+            for (int x = 0; x < 3; ++x) out[9 * z + 3 * y + x] += rz.r0[z] * P[y][x] + rz.r1[z] * W[y][x];
+}
+
+// out_q += sum_{alpha<=beta} A_{alpha beta} R^{alpha beta}_q(u): second-order central moments
+template <typename real>
+__device__ __forceinline__ void add_second_order27(real Axx, real Ayy, real Azz, real Axy, real Axz, real Ayz, const R1D<real>& rx,
+                                                   const R1D<real>& ry, const R1D<real>& rz, real out[27]) {
+    const real r2[3] = {real(0.5), real(-1), real(0.5)};
+    real P[3][3], Qm[3][3], W[3][3];
+#pragma unroll
+    for (int y = 0; y < 3; ++y)
+#pragma unroll
+        for (int x = 0; x < 3; ++x) {
+            P[y][x] = Axx * r2[x] * ry.r0[y] + Ayy * rx.r0[x] * r2[y] + Axy * rx.r1[x] * ry.r1[y];
+            Qm[y][x] = Axz * rx.r1[x] * ry.r0[y] + Ayz * rx.r0[x] * ry.r1[y];
+            W[y][x] = Azz * rx.r0[x] * ry.r0[y];
+        }
+#pragma unroll
+    for (int z = 0; z < 3; ++z)
+#pragma unroll
+        for (int y = 0; y < 3; ++y)
+#pragma unroll
+            for (int x = 0; x < 3; ++x)
+                out[9 * z + 3 * y + x] += rz.r0[z] * P[y][x] + rz.r1[z] * Qm[y][x] + r2[z] * W[y][x];
+}
+
+}  // namespace tcp

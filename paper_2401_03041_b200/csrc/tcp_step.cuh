@@ -1,0 +1,323 @@
+// The kernels proper (see tcp_kernels.cuh for the overview).
+#pragma once
+#include "tcp_kernels.cuh"
+
+namespace tcp {
+
+constexpr int kBlock = 128;
+
+// fp32 only.  In real arithmetic the collision conserves the zeroth moment (sum_q E_q = s because
+// sum_q w_q = 1), but the rounded weights do not sum to 1, which re-creates the whole population
+// with the same relative bias (~1e-8) every step: sum(phi) then drifts linearly (measured 7.5e-5
+// over 1e4 steps).  So the zeroth moment of the pulled populations is summed in fp64 (exact for 27
+// floats of similar size) and the rest population is written as the fp64 remainder, rounded once:
+// what is left is one unbiased rounding per cell and step.  In fp64 the bias is ~1e-17 per step
+// and the arithmetic is left as derived.
+template <typename real>
+__device__ __forceinline__ double exact_sum27(const real a[27]) {
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 27; ++q) s += (double)a[q];
+    return s;
+}
+template <typename real>
+__device__ __forceinline__ void conserve_zeroth27(real a[27], double s) {
+    if constexpr (sizeof(real) == 4) {
+#pragma unroll
+        for (int q = 0; q < 27; ++q)
+            if (q != 13) s -= (double)a[q];
+        a[13] = (real)s;
+    }
+}
+
+// ---- phase-field LB on one cell: eqs. 10-15 ---------------------------------------------------
+// h = pulled populations; G = grad phi^n, phi_c = phi^n (interface force from the stored phi,
+// reading S10); un = u^n.  Writes h~ and phi' = sum h (eq. 13).
+template <typename real, bool BGK>
+__device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27], const real G[3], real phi_c, const real un[3]) {
+    const Mom2<real> M = moments27<real, false>(h);
+    double phin_exact = 0.0;
+    if constexpr (sizeof(real) == 4) phin_exact = exact_sum27<real>(h);
+    const real phin = sizeof(real) == 4 ? (real)phin_exact : M.m0;
+    // a = c_s^2 [4 phi (1 - phi) / xi] n,  n = G / sqrt(G.G + eps)   (eq. 15, readings S7, S8)
+    const real inv = rsqrt_<real>(G[0] * G[0] + G[1] * G[1] + G[2] * G[2] + A.eps);
+    const real mag = real(4.0 / 3.0) * phi_c * (real(1) - phi_c) / A.xi * inv;
+    real a[3] = {mag * G[0], mag * G[1], mag * G[2]};
+    const real w = A.w_phi;
+    if (BGK) {   // a~ = (1-w) a + w [a_eq + F(a (2-w)/w)/2]
+        const real sc = (real(2) - w) / w;
+        a[0] *= sc; a[1] *= sc; a[2] *= sc;
+    }
+    real b[3], v[3];
+#pragma unroll
+    for (int al = 0; al < 3; ++al) { b[al] = phin * un[al] + a[al]; v[al] = phin * un[al] + real(0.5) * a[al]; }
+    const real A0 = phin - real(1.5) * (un[0] * b[0] + un[1] * b[1] + un[2] * b[2]);
+    real out[27];
+    equilibrium_plus_half_force27<real>(A0, un, v, b, out);
+    if (BGK) {
+#pragma unroll
+        for (int q = 0; q < 27; ++q) h[q] = (real(1) - w) * h[q] + w * out[q];
+    } else {
+        // first-order central moments of (h - h_eq) + F/2 relax with w_phi, everything else with 1
+        const real k1 = real(1) - w;
+        const real m[3] = {k1 * ((M.mx - phin * un[0]) + real(0.5) * a[0]),
+                           k1 * ((M.my - phin * un[1]) + real(0.5) * a[1]),
+                           k1 * ((M.mz - phin * un[2]) + real(0.5) * a[2])};
+        R1D<real> rx, ry, rz;
+        rx.set(un[0]); ry.set(un[1]); rz.set(un[2]);
+        add_first_order27<real>(m, rx, ry, rz, out);
+#pragma unroll
+        for (int q = 0; q < 27; ++q) h[q] = out[q];
+    }
+    conserve_zeroth27<real>(h, phin_exact);
+    return phin;
+}
+
+// ---- hydrodynamic LB on one cell: eqs. 16-22, forces of eqs. 7-9 -------------------------------
+// g = pulled populations; phi_c, G, lapPhi from phi^n (S16); T_c, Th = grad T^n.  Writes g~, u^{n+1}.
+template <typename real, bool BGK>
+__device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27], real phi_c, const real G[3], real lapPhi,
+                                              real T_c, const real Th[3], real u[3]) {
+    const Mom2<real> M = moments27<real, true>(g);
+    double ps_exact = 0.0;
+    if constexpr (sizeof(real) == 4) ps_exact = exact_sum27<real>(g);
+    const real ps = sizeof(real) == 4 ? (real)ps_exact : M.m0;   // p* (eq. 17)
+    const real j[3] = {M.mx, M.my, M.mz};
+    const real rho = A.rho_L + phi_c * A.drho;              // eq. 14
+    const real tau = A.tau_L + phi_c * A.dtau;              // eq. 22
+    const real sigma = A.sigma_ref + A.sigma_T * (T_c - A.T_ref);   // eq. 9
+    // mu_phi = 4 beta phi (phi-1)(phi-1/2) - k lap phi, beta = 12 sigma/xi, k = 3 sigma xi/2  (S5)
+    const real mu = real(48) * sigma / A.xi * phi_c * (phi_c - real(1)) * (phi_c - real(0.5)) - real(1.5) * sigma * A.xi * lapPhi;
+    const real GG = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
+    const real TG = Th[0] * G[0] + Th[1] * G[1] + Th[2] * G[2];
+    const real mar = real(1.5) * A.xi * A.sigma_T;          // eq. 8 (with |grad phi|^2, G2)
+    const real pcoef = ps * real(1.0 / 3.0) * A.drho;       // eq. 20
+    const real i2r = real(0.5) / rho;
+    real F[3], us[3];
+#pragma unroll
+    for (int al = 0; al < 3; ++al) {
+        F[al] = mu * G[al] + mar * (GG * Th[al] - TG * G[al]) + rho * A.grav[al] - pcoef * G[al];
+        us[al] = j[al] + F[al] * i2r;                       // predictor u* (S4)
+    }
+    const real om = real(1) / (tau + real(0.5));
+    {   // F_mu = -(tau/(tau+1/2)) (rho_H - rho_L) Pi* . G, Pi* = sum c c (g - g_eq(p*, u*))  (eq. 21)
+        const real p3 = ps * real(1.0 / 3.0);
+        const real Pxx = M.mxx - (p3 + us[0] * us[0]), Pyy = M.myy - (p3 + us[1] * us[1]), Pzz = M.mzz - (p3 + us[2] * us[2]);
+        const real Pxy = M.mxy - us[0] * us[1], Pxz = M.mxz - us[0] * us[2], Pyz = M.myz - us[1] * us[2];
+        const real cf = -(tau * om) * A.drho;
+        F[0] += cf * (Pxx * G[0] + Pxy * G[1] + Pxz * G[2]);
+        F[1] += cf * (Pxy * G[0] + Pyy * G[1] + Pyz * G[2]);
+        F[2] += cf * (Pxz * G[0] + Pyz * G[1] + Pzz * G[2]);
+    }
+    real a[3], d[3];
+#pragma unroll
+    for (int al = 0; al < 3; ++al) {
+        d[al] = -F[al] * i2r;                               // j - u
+        u[al] = j[al] + F[al] * i2r;                        // u^{n+1} (S6)
+        a[al] = real(2) * F[al] * i2r;                      // Guo vector F / rho
+    }
+    if (BGK) {
+        const real sc = (real(2) - om) / om;
+        a[0] *= sc; a[1] *= sc; a[2] *= sc;
+    }
+    real b[3], v[3];
+#pragma unroll
+    for (int al = 0; al < 3; ++al) { b[al] = u[al] + a[al]; v[al] = u[al] + real(0.5) * a[al]; }
+    const real A0 = ps - real(1.5) * (u[0] * b[0] + u[1] * b[1] + u[2] * b[2]);
+    real out[27];
+    equilibrium_plus_half_force27<real>(A0, u, v, b, out);
+    if (BGK) {
+#pragma unroll
+        for (int q = 0; q < 27; ++q) g[q] = (real(1) - om) * g[q] + om * out[q];
+    } else {
+        // second-order central moments of g - g_eq: deviatoric part relaxes with omega, trace with
+        // s_bulk, everything else with 1 (reading S2); Guo populations have none
+        const real p3 = ps * real(1.0 / 3.0);
+        real kxx = M.mxx - (p3 + u[0] * u[0]) - real(2) * u[0] * d[0];
+        real kyy = M.myy - (p3 + u[1] * u[1]) - real(2) * u[1] * d[1];
+        real kzz = M.mzz - (p3 + u[2] * u[2]) - real(2) * u[2] * d[2];
+        const real kxy = M.mxy - u[0] * u[1] - u[0] * d[1] - u[1] * d[0];
+        const real kxz = M.mxz - u[0] * u[2] - u[0] * d[2] - u[2] * d[0];
+        const real kyz = M.myz - u[1] * u[2] - u[1] * d[2] - u[2] * d[1];
+        const real tr3 = (kxx + kyy + kzz) * real(1.0 / 3.0);
+        const real k2 = real(1) - om, kb = (real(1) - A.s_bulk) * tr3;
+        kxx = k2 * (kxx - tr3) + kb; kyy = k2 * (kyy - tr3) + kb; kzz = k2 * (kzz - tr3) + kb;
+        R1D<real> rx, ry, rz;
+        rx.set(u[0]); ry.set(u[1]); rz.set(u[2]);
+        add_second_order27<real>(kxx, kyy, kzz, k2 * kxy, k2 * kxz, k2 * kyz, rx, ry, rz, out);
+#pragma unroll
+        for (int q = 0; q < 27; ++q) g[q] = out[q];
+    }
+    conserve_zeroth27<real>(g, ps_exact);
+}
+
+// ---- thermal LB on one cell: eqs. 27-29 (rho c_p = 1 on this path, S11) ------------------------
+template <typename real, int Q, bool BGK>
+__device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[Q], real phi_new, const real u[3], real qT) {
+    real Tn = real(0), j[3] = {real(0), real(0), real(0)};
+    double Tn_exact = 0.0;
+    static_for<0, Q>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(Q, k);
+        if constexpr (sizeof(real) == 4) Tn_exact += (double)f[k]; else
+        Tn += f[k];                                          // eq. 28
+        if constexpr (cx27(q) != 0) j[0] += real(cx27(q)) * f[k];
+        if constexpr (cy27(q) != 0) j[1] += real(cy27(q)) * f[k];
+        if constexpr (cz27(q) != 0) j[2] += real(cz27(q)) * f[k];
+    });
+    if constexpr (sizeof(real) == 4) Tn = (real)Tn_exact;
+    const real kap = A.kappa_L + phi_new * A.dkappa;         // eq. 23 (G5)
+    const real w = real(1) / (real(0.5) + real(3) * kap);    // eq. 29 read as a rate (G4)
+    real out[Q];
+    thermal_equilibrium<real, Q>(Tn, u, out);
+    if (BGK) {
+        static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; out[k] = (real(1) - w) * f[k] + w * out[k]; });
+    } else {
+        const real k1 = real(1) - w;
+        const real m[3] = {k1 * (j[0] - Tn * u[0]), k1 * (j[1] - Tn * u[1]), k1 * (j[2] - Tn * u[2])};
+        if constexpr (Q == 27) {
+            R1D<real> rx, ry, rz;
+            rx.set(u[0]); ry.set(u[1]); rz.set(u[2]);
+            add_first_order27<real>(m, rx, ry, rz, out);
+        } else {
+            add_first_order_thermal<real, Q>(m, u, out);
+        }
+    }
+    if constexpr (sizeof(real) == 4) {   // see conserve_zeroth27
+        double rest = Tn_exact;
+        static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; if constexpr (k != Q / 2) rest -= (double)out[k]; });
+        out[Q / 2] = (real)rest;
+    }
+    static_for<0, Q>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(Q, k);
+        f[k] = out[k] + real(weight(Q, cls27(q))) * qT;      // + w_i q_T (eq. 27)
+    });
+    return Tn;
+}
+
+// ---------------------------------------------------------------------------------------------
+template <typename real, int QT, bool WALLS, bool BGK>
+__global__ void __launch_bounds__(kBlock) fused_step_kernel(const StepArgs<real> A) {
+    const int cell = blockIdx.x * kBlock + threadIdx.x;
+    if (cell >= A.ncell) return;
+    const long long N = A.ncell;
+    Nbh<WALLS> nb;
+    nb.init(A, cell);
+
+    real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
+    stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
+    stencil27<real, WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
+    real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
+
+    real phi_new;
+    {
+        real h[27];
+        pull27<real, WALLS>(A, nb, A.h_in, h);
+        phi_new = collide_phase<real, BGK>(A, h, G, phi_c, u);
+#pragma unroll
+        for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = h[q];
+        A.phi_out[cell] = phi_new;
+    }
+    {
+        real g[27];
+        pull27<real, WALLS>(A, nb, A.g_in, g);
+        collide_hydro<real, BGK>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+#pragma unroll
+        for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
+        A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
+    }
+    if constexpr (QT > 0) {
+        real f[QT];
+        pull_thermal<real, QT, WALLS>(A, nb, A.f_in, f);
+        const real qT = A.q_src ? A.q_src[cell] : real(0);
+        const real Tn = collide_thermal<real, QT, BGK>(A, f, phi_new, u, qT);
+        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
+        A.T_out[cell] = Tn;
+    }
+}
+
+// ---- Runge-Kutta stages of eq. 4 (eqs. 25-26; reading G6) --------------------
+template <typename real>
+struct RkArgs {
+    StepArgs<real> S;        // geometry, walls, phi_in = phi^{n+1}, u = u^{n+1}, q_src
+    const real* Y;           // stage field (differentiated)
+    const real* Tn;          // T^n
+    const real* acc_in;      // RK4 accumulator
+    real* out;               // next stage field / T^{n+1}
+    real* acc_out;
+    real c_out;              // out = Tn + c_out R      (stages 1-3; RK2 stage 2)
+    real c_acc;              // acc_out = (first ? Tn : acc_in) + c_acc R
+    int mode;                // 0: out only; 1: out and acc from Tn; 2: out and acc from acc_in; 3: out = acc_in + c_acc R
+};
+
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(kBlock) rk_stage_kernel(const RkArgs<real> R) {
+    const StepArgs<real>& A = R.S;
+    const int cell = blockIdx.x * kBlock + threadIdx.x;
+    if (cell >= A.ncell) return;
+    const long long N = A.ncell;
+    Nbh<WALLS> nb;
+    nb.init(A, cell);
+    real phi_c, G[3], lapPhi, Y_c, gY[3], lapY;
+    stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
+    stencil27<real, WALLS, true>(A, nb, R.Y, Y_c, gY, lapY);
+    const real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
+    const real kap = A.kappa_L + phi_c * A.dkappa;
+    const real rcp = (A.rho_L + phi_c * A.drho) * (A.cp_L + phi_c * A.dcp);   // rho(phi) c_p(phi) (A14)
+    const real adv = u[0] * gY[0] + u[1] * gY[1] + u[2] * gY[2];
+    const real dk = A.dkappa * (G[0] * gY[0] + G[1] * gY[1] + G[2] * gY[2]);
+    const real rhs = -adv + (dk + kap * lapY) / rcp + (A.q_src ? A.q_src[cell] : real(0));
+    const real Tn = R.Tn[cell];
+    if (R.mode == 3) {
+        R.out[cell] = R.acc_in[cell] + R.c_acc * rhs;
+    } else {
+        R.out[cell] = Tn + R.c_out * rhs;
+        if (R.mode == 1) R.acc_out[cell] = Tn + R.c_acc * rhs;
+        if (R.mode == 2) R.acc_out[cell] = R.acc_in[cell] + R.c_acc * rhs;
+    }
+}
+
+// ---- initialisation and read-back --------------------------------------------------------------
+template <typename real, int QT>
+__global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
+    const int cell = blockIdx.x * kBlock + threadIdx.x;
+    if (cell >= A.ncell) return;
+    const long long N = A.ncell;
+    const real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
+    const real uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    real out[27];
+    {
+        const real s = A.phi_in[cell];
+        const real su[3] = {s * u[0], s * u[1], s * u[2]};
+        equilibrium_plus_half_force27<real>(s - real(1.5) * s * uu, u, su, su, out);      // eq. 12
+#pragma unroll
+        for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = out[q];
+    }
+    equilibrium_plus_half_force27<real>(-real(1.5) * uu, u, u, u, out);                   // eq. 18, p* = 0
+#pragma unroll
+    for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = out[q];
+    if constexpr (QT > 0) {
+        real f[QT];
+        thermal_equilibrium<real, QT>(A.T_in[cell], u, f);
+        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
+    }
+}
+
+template <typename real>
+__global__ void __launch_bounds__(kBlock) pressure_kernel(const real* __restrict__ g, const real* __restrict__ phi, real* __restrict__ p,
+                                                         int ncell, real rho_L, real drho) {
+    const int cell = blockIdx.x * kBlock + threadIdx.x;
+    if (cell >= ncell) return;
+    const long long N = ncell;
+    real s = real(0);
+#pragma unroll
+    for (int q = 0; q < 27; ++q) s += g[q * N + cell];
+    p[cell] = real(1.0 / 3.0) * (rho_L + phi[cell] * drho) * s;
+}
+
+template <typename real>
+__global__ void fill_kernel(real* __restrict__ a, long long n, real v) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] = v;
+}
+
+}  // namespace tcp

@@ -4,7 +4,15 @@
 
 namespace tcp {
 
-constexpr int kBlock = 128;
+#ifndef TCP_BLOCK
+#define TCP_BLOCK 128
+#endif
+// 3 resident blocks of 128 threads per SM (168 registers per thread, ~90 B of spills in fp64) measured
+// 5 % faster than 2 blocks at 248 registers; 4 blocks (128 registers) spill too much (profiles/).
+#ifndef TCP_MINB
+#define TCP_MINB 3
+#endif
+constexpr int kBlock = TCP_BLOCK;
 
 // fp32 only.  In real arithmetic the collision conserves the zeroth moment (sum_q E_q = s because
 // sum_q w_q = 1), but the rounded weights do not sum to 1, which re-creates the whole population
@@ -196,7 +204,7 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
 
 // ---------------------------------------------------------------------------------------------
 template <typename real, int QT, bool WALLS, bool BGK>
-__global__ void __launch_bounds__(kBlock) fused_step_kernel(const StepArgs<real> A) {
+__global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const StepArgs<real> A) {
     const int cell = blockIdx.x * kBlock + threadIdx.x;
     if (cell >= A.ncell) return;
     const long long N = A.ncell;

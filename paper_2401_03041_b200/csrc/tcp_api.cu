@@ -8,7 +8,9 @@
 #include <new>
 
 #include "../../include/tcp.h"
-#include "tcp_step.cuh"
+#include <cstdlib>
+
+#include "tcp_rows.cuh"
 
 namespace {
 
@@ -108,6 +110,11 @@ struct tcp_sim {
     bool initialised, has_q, walls, stepped;
     long long launches;
     cudaEvent_t ev0, ev1;
+    bool use_async;          // cp.async staged kernel
+    int bz;                  // z-slab thickness of the cell visiting order
+    bool use_rows;           // TMA row-segment kernel eligible (x periodic, nx % (16 B / element) == 0, not BGK)
+    int rows_L, rows_threads;
+    size_t rows_smem;
 };
 
 namespace {
@@ -121,6 +128,7 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     const tcp_params& P = s->P;
     const int c = s->cur, o = 1 - s->cur;
     A.nx = s->nx; A.ny = s->ny; A.nz = s->nz; A.ncell = (int)s->N;
+    A.bz = s->bz;
     for (int a = 0; a < 3; ++a) A.wall[a] = P.bc[a] == TCP_BC_WALLS;
     A.h_in = ptr<real>(s, s->L.h[c]); A.h_out = ptr<real>(s, s->L.h[o]);
     A.g_in = ptr<real>(s, s->L.g[c]); A.g_out = ptr<real>(s, s->L.g[o]);
@@ -160,11 +168,54 @@ void launch_fused(const tcp_sim* s, const tcp::StepArgs<real>& A) {
     }
 }
 
+template <typename real, bool WALLS, bool BGK>
+int launch_async(const tcp_sim* s, const tcp::StepArgs<real>& A) {
+    const unsigned grid = grid_for(s->N);
+    const int QT = thermal_q(s->P.thermal);
+    const size_t smem = (size_t)(54 + QT) * tcp::kBlock * sizeof(real);
+#define TCP_ASYNC_LAUNCH(Q)                                                                               \
+    do {                                                                                                  \
+        auto kern = tcp::fused_step_async_kernel<real, Q, WALLS, BGK>;                                    \
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));           \
+        kern<<<grid, tcp::kBlock, smem, s->stream>>>(A);                                                  \
+    } while (0)
+    switch (QT) {
+    case 7: TCP_ASYNC_LAUNCH(7); break;
+    case 15: TCP_ASYNC_LAUNCH(15); break;
+    case 19: TCP_ASYNC_LAUNCH(19); break;
+    case 27: TCP_ASYNC_LAUNCH(27); break;
+    default: TCP_ASYNC_LAUNCH(0); break;
+    }
+#undef TCP_ASYNC_LAUNCH
+    return TCP_OK;
+}
+
 template <typename real>
 void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
     const unsigned grid = grid_for(s->N);
     if (s->walls) tcp::rk_stage_kernel<real, true><<<grid, tcp::kBlock, 0, s->stream>>>(R);
     else tcp::rk_stage_kernel<real, false><<<grid, tcp::kBlock, 0, s->stream>>>(R);
+}
+
+template <typename real, bool WALLS>
+int launch_rows(const tcp_sim* s, const tcp::StepArgs<real>& A) {
+    const dim3 grid((unsigned)((s->nx + s->rows_L - 1) / s->rows_L), (unsigned)s->ny, (unsigned)s->nz);
+    const dim3 block((unsigned)s->rows_threads);
+#define TCP_ROWS_LAUNCH(Q)                                                                                         \
+    do {                                                                                                           \
+        auto kern = tcp::fused_step_rows_kernel<real, Q, WALLS>;                                                  \
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->rows_smem));           \
+        kern<<<grid, block, s->rows_smem, s->stream>>>(A, s->rows_L);                                             \
+    } while (0)
+    switch (thermal_q(s->P.thermal)) {
+    case 7: TCP_ROWS_LAUNCH(7); break;
+    case 15: TCP_ROWS_LAUNCH(15); break;
+    case 19: TCP_ROWS_LAUNCH(19); break;
+    case 27: TCP_ROWS_LAUNCH(27); break;
+    default: TCP_ROWS_LAUNCH(0); break;
+    }
+#undef TCP_ROWS_LAUNCH
+    return TCP_OK;
 }
 
 // one time step: Algorithm 1 (thermal LB, one fused kernel) or Algorithm 2 (fused phase+hydro
@@ -173,8 +224,15 @@ template <typename real>
 int step_once(tcp_sim* s) {
     tcp::StepArgs<real> A = make_args<real>(s);
     const bool bgk = s->P.high_rate_equals_shear != 0;
-    if (s->walls) { if (bgk) launch_fused<real, true, true>(s, A); else launch_fused<real, true, false>(s, A); }
-    else          { if (bgk) launch_fused<real, false, true>(s, A); else launch_fused<real, false, false>(s, A); }
+    if (s->use_async) {
+        int rc = s->walls ? (bgk ? launch_async<real, true, true>(s, A) : launch_async<real, true, false>(s, A))
+                          : (bgk ? launch_async<real, false, true>(s, A) : launch_async<real, false, false>(s, A));
+        if (rc) return rc;
+    } else if (s->use_rows) {
+        int rc = s->walls ? launch_rows<real, true>(s, A) : launch_rows<real, false>(s, A);
+        if (rc) return rc;
+    } else if (s->walls) { if (bgk) launch_fused<real, true, true>(s, A); else launch_fused<real, true, false>(s, A); }
+    else                 { if (bgk) launch_fused<real, false, true>(s, A); else launch_fused<real, false, false>(s, A); }
     s->launches++;
     const int th = s->P.thermal;
     if (th == TCP_THERMAL_RK2 || th == TCP_THERMAL_RK4) {
@@ -291,6 +349,26 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
     s->L = make_layout(nx, ny, nz, p);
     s->walls = p->bc[0] == TCP_BC_WALLS || p->bc[1] == TCP_BC_WALLS || p->bc[2] == TCP_BC_WALLS;
     s->owns_memory = own; s->owns_stream = own;
+    {   // kernel choice: the TMA row-segment kernel where its alignment rules hold (tcp_rows.cuh), else the flat one.
+        // TCP_KERNEL=flat / rows overrides (tuning and A/B tests); TCP_ROWS_L sets the segment length.
+        const int es = p->precision == TCP_F64 ? 8 : 4, AH = 16 / es;
+        const char* force = std::getenv("TCP_KERNEL");
+        s->use_rows = p->bc[0] == TCP_BC_PERIODIC && nx % AH == 0 && !p->high_rate_equals_shear;
+        s->bz = 1;   // measured at 400^3: slabs of 8 / 16 / 32 planes are 2-3 % SLOWER than plain z order (profiles/r01_notes.md)
+        if (const char* b = std::getenv("TCP_BZ")) { int v = std::atoi(b); if (v >= 1) s->bz = v < nz ? v : nz; }
+        // default: the cp.async staged kernel; TCP_KERNEL=flat (register-staged) / rows (TMA bulk rows) for A/B runs
+        s->use_async = !force || std::strcmp(force, "async") == 0;
+        if (!force || std::strcmp(force, "rows") != 0) s->use_rows = false;
+        int cap = tcp::kRowsMaxThreads;
+        if (const char* l = std::getenv("TCP_ROWS_L")) { int v = std::atoi(l); if (v >= AH && v <= cap) cap = v; }
+        const int nseg = (nx + cap - 1) / cap;
+        int L = (nx + nseg - 1) / nseg;
+        L = (L + AH - 1) / AH * AH;
+        s->rows_L = L;
+        s->rows_threads = (L + 31) / 32 * 32;
+        s->rows_smem = (size_t)(54 + thermal_q(p->thermal)) * (L + 2 * AH) * es + 64;
+        if (s->rows_smem > 200 * 1024) s->use_rows = false;
+    }
     if (own) {
         void* mem = nullptr;
         e = cudaMalloc(&mem, s->L.total);

@@ -205,11 +205,12 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
 // ---------------------------------------------------------------------------------------------
 template <typename real, int QT, bool WALLS, bool BGK>
 __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const StepArgs<real> A) {
-    const int cell = blockIdx.x * kBlock + threadIdx.x;
-    if (cell >= A.ncell) return;
+    const int gtid = blockIdx.x * kBlock + threadIdx.x;
+    if (gtid >= A.ncell) return;
     const long long N = A.ncell;
     Nbh<WALLS> nb;
-    nb.init(A, cell);
+    nb.init(A, gtid);
+    const int cell = nb.idx;
 
     real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
     stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
@@ -243,6 +244,114 @@ __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const Step
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// fused_step_async_kernel: the same step, but every thread first issues ALL of its 27 + 27 + Q_T
+// pulls as asynchronous global->shared copies (cp.async, SASS LDGSTS; slot [q][tid], so a thread only
+// ever reads what it copied itself and cp.async.wait_group is the only synchronisation needed), then
+// does the phi / T stencils, then consumes the three groups in order.  Loads in flight per SM become
+// blocks x 128 x (54 + Q_T) x sizeof(real) (187 KB in fp64) instead of whatever the register
+// allocator manages to hoist; registers no longer hold prefetched populations.
+template <typename real>
+__device__ __forceinline__ void cp_async_elem(real* smem_dst, const real* gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    if constexpr (sizeof(real) == 8)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <typename real, int QT, bool WALLS, bool BGK>
+__global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_async_kernel(const StepArgs<real> A) {
+    extern __shared__ __align__(16) unsigned char smem_raw_async[];
+    real* stage = reinterpret_cast<real*>(smem_raw_async);     // [54 + QT][kBlock]
+    const int tid = threadIdx.x;
+    const int gtid = blockIdx.x * kBlock + tid;
+    const bool active = gtid < A.ncell;
+    const long long N = A.ncell;
+    Nbh<WALLS> nb;
+    nb.init(A, active ? gtid : A.ncell - 1);                   // tail lanes shadow the last cell, store nothing
+    const int cell = nb.idx;
+
+    // issue every pull of this cell (bounce-back links copy the opposite direction of the own cell)
+#pragma unroll
+    for (int q = 0; q < 27; ++q) {
+        int face = 0;
+        const bool bb = WALLS && nb.crossed(-cx27(q), -cy27(q), -cz27(q), face) >= 0;
+        cp_async_elem<real>(stage + q * kBlock + tid, bb ? A.h_in + (26 - q) * N + cell : A.h_in + q * N + nb.at(-cx27(q), -cy27(q), -cz27(q)));
+    }
+    cp_async_commit();
+#pragma unroll
+    for (int q = 0; q < 27; ++q) {
+        int face = 0;
+        const bool bb = WALLS && nb.crossed(-cx27(q), -cy27(q), -cz27(q), face) >= 0;
+        cp_async_elem<real>(stage + (27 + q) * kBlock + tid, bb ? A.g_in + (26 - q) * N + cell : A.g_in + q * N + nb.at(-cx27(q), -cy27(q), -cz27(q)));
+    }
+    cp_async_commit();
+    if constexpr (QT > 0) {
+        static_for<0, QT>([&](auto K) {
+            constexpr int k = decltype(K)::value, q = q_of(QT, k);
+            int face = 0;
+            const bool bb = WALLS && nb.crossed(-cx27(q), -cy27(q), -cz27(q), face) >= 0;
+            cp_async_elem<real>(stage + (54 + k) * kBlock + tid,
+                                bb ? A.f_in + (QT - 1 - k) * N + cell : A.f_in + k * N + nb.at(-cx27(q), -cy27(q), -cz27(q)));
+        });
+    }
+    cp_async_commit();
+
+    real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
+    stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
+    stencil27<real, WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
+    real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
+
+    real phi_new;
+    {
+        cp_async_wait<2>();
+        real h[27];
+#pragma unroll
+        for (int q = 0; q < 27; ++q) h[q] = stage[q * kBlock + tid];
+        phi_new = collide_phase<real, BGK>(A, h, G, phi_c, u);
+        if (active) {
+#pragma unroll
+            for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = h[q];
+            A.phi_out[cell] = phi_new;
+        }
+    }
+    {
+        cp_async_wait<1>();
+        real g[27];
+#pragma unroll
+        for (int q = 0; q < 27; ++q) g[q] = stage[(27 + q) * kBlock + tid];
+        collide_hydro<real, BGK>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+        if (active) {
+#pragma unroll
+            for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
+            A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
+        }
+    }
+    if constexpr (QT > 0) {
+        cp_async_wait<0>();
+        real f[QT];
+        static_for<0, QT>([&](auto K) {
+            constexpr int k = decltype(K)::value, q = q_of(QT, k);
+            int face = 0;
+            const int ax = nb.crossed(-cx27(q), -cy27(q), -cz27(q), face);
+            const real v = stage[(54 + k) * kBlock + tid];
+            if (WALLS && ax >= 0)   // anti-bounce-back (S9): the staged value is f~_opp of the own cell
+                f[k] = real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, -cx27(q), -cy27(q), -cz27(q)) - v;
+            else
+                f[k] = v;
+        });
+        const real qT = A.q_src ? A.q_src[cell] : real(0);
+        const real Tn = collide_thermal<real, QT, BGK>(A, f, phi_new, u, qT);
+        if (active) {
+            static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
+            A.T_out[cell] = Tn;
+        }
+    }
+}
+
 // ---- Runge-Kutta stages of eq. 4 (eqs. 25-26; reading G6) --------------------
 template <typename real>
 struct RkArgs {
@@ -260,11 +369,12 @@ struct RkArgs {
 template <typename real, bool WALLS>
 __global__ void __launch_bounds__(kBlock) rk_stage_kernel(const RkArgs<real> R) {
     const StepArgs<real>& A = R.S;
-    const int cell = blockIdx.x * kBlock + threadIdx.x;
-    if (cell >= A.ncell) return;
+    const int gtid = blockIdx.x * kBlock + threadIdx.x;
+    if (gtid >= A.ncell) return;
     const long long N = A.ncell;
     Nbh<WALLS> nb;
-    nb.init(A, cell);
+    nb.init(A, gtid);
+    const int cell = nb.idx;
     real phi_c, G[3], lapPhi, Y_c, gY[3], lapY;
     stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
     stencil27<real, WALLS, true>(A, nb, R.Y, Y_c, gY, lapY);

@@ -258,6 +258,39 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: MLUPS and HBM-roofline fraction for each thermal variant and size.
+    One JSON line per (size, precision, variant); device-resident timing only.  Not the driver's line."""
+    import paper_2401_03041_b200 as tcp
+    torch.cuda.set_device(0)
+    peak, peak_src = hbm_peak()
+    cases = [(n, "f64") for n in (128, 192, 256, 320, 400)] + [(512, "f32")]
+    if args.sweep_sizes:
+        cases = [(int(t.split(":")[0]), t.split(":")[1] if ":" in t else "f64") for t in args.sweep_sizes.split(",")]
+    for n, prec in cases:
+        es = 8 if prec == "f64" else 4
+        tdt = torch.float64 if prec == "f64" else torch.float32
+        for thermal in ("lb_d3q7", "lb_d3q15", "lb_d3q19", "lb_d3q27", "rk2", "rk4"):
+            wl = W.perf_box(n, thermal=thermal, device="cuda")
+            sim = tcp.Simulation(n, n, n, dict(wl.params, precision=prec))
+            sim.init_fields(wl.phi.to(tdt).contiguous(), None, wl.T.to(tdt).contiguous())
+            sim.step(max(args.warmup, 3))
+            times = []
+            for _ in range(5):
+                sim.step(args.steps)
+                times.append(sim.last_step_ms() / args.steps)
+            ms = statistics.median(times)
+            finite = bool(torch.isfinite(sim.read_fields_device()[0]).all().item())
+            sim.close()
+            bpc = step_values_per_cell(thermal) * es
+            gbs = bpc * n ** 3 / (ms * 1e-3) / 1e9
+            print(json.dumps({"sweep": True, "size": n, "dtype": prec, "thermal": thermal, "ms_per_step": ms,
+                              "mlups": n ** 3 / (ms * 1e-3) / 1e6, "step_bytes_per_cell": bpc, "gbs": gbs,
+                              "frac_of_measured_peak": gbs / peak, "finite": finite}), flush=True)
+            del sim, wl
+            torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -270,10 +303,14 @@ def main():
     ap.add_argument("--ref-size", type=int, default=40)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="per-variant / per-size table (configs[4]); one JSON line each")
+    ap.add_argument("--sweep-sizes", default="", help="e.g. 256:f64,512:f32")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: W >= 3
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -262,8 +262,15 @@ __device__ __forceinline__ void cp_async_elem(real* smem_dst, const real* gsrc) 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// Residency: (54 + Q_T) x 128 x sizeof(real) bytes of staging per block.  In fp64 three blocks of the
+// D3Q15 / D3Q19 variants would take 212-224 KB of the SM's 256 KB, leaving almost no L1 for the
+// phi / T stencil loads (measured 0.65 of the HBM peak against 0.81-0.84 for D3Q7 and for D3Q27, which
+// only fits two blocks anyway), so those are compiled for two blocks per SM.
+template <typename real, int QT>
+constexpr int async_min_blocks() { return (sizeof(real) == 8 && QT >= 15) ? 2 : TCP_MINB; }
+
 template <typename real, int QT, bool WALLS, bool BGK>
-__global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_async_kernel(const StepArgs<real> A) {
+__global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_step_async_kernel(const StepArgs<real> A) {
     extern __shared__ __align__(16) unsigned char smem_raw_async[];
     real* stage = reinterpret_cast<real*>(smem_raw_async);     // [54 + QT][kBlock]
     const int tid = threadIdx.x;

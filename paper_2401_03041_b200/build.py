@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtcp.so")
 SOURCES = ["tcp_api.cu"]
-HEADERS = ["tcp_lattice.cuh", "tcp_device.cuh", "tcp_kernels.cuh", "tcp_step.cuh", "tcp_rows.cuh"]
+HEADERS = ["tcp_lattice.cuh", "tcp_device.cuh", "tcp_kernels.cuh", "tcp_step.cuh", "tcp_rows.cuh", "tcp_rk.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "--use_fast_math" if False else "-fmad=true",   # IEEE division / sqrt kept; FMA contraction on
               "-Xcompiler", "-fPIC", "-shared"]

@@ -10,6 +10,7 @@
 #include "../../include/tcp.h"
 #include <cstdlib>
 
+#include "tcp_rk.cuh"
 #include "tcp_rows.cuh"
 
 namespace {
@@ -53,6 +54,7 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
     if (p->struct_size != sizeof(tcp_params)) return fail(TCP_EINVAL, "tcp_params.struct_size != sizeof(tcp_params)");
     if (nx < 1 || ny < 1 || nz < 1) return fail(TCP_EINVAL, "extents must be >= 1");
     if ((double)nx * ny * nz >= 2147483647.0) return fail(TCP_EINVAL, "nx*ny*nz must be < 2^31");
+    if (ny > 65535 * 8 || nz > 65535) return fail(TCP_EINVAL, "ny must be <= 524280 and nz <= 65535 (grid limits)");
     const int n[3] = {nx, ny, nz};
     for (int a = 0; a < 3; ++a) {
         if (p->bc[a] != TCP_BC_PERIODIC && p->bc[a] != TCP_BC_WALLS) return fail(TCP_EINVAL, "bc must be TCP_BC_PERIODIC or TCP_BC_WALLS");
@@ -192,6 +194,13 @@ int launch_async(const tcp_sim* s, const tcp::StepArgs<real>& A) {
 
 template <typename real>
 void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
+    if (s->use_async) {   // default: z-marching tile kernel (tcp_rk.cuh)
+        const dim3 block(tcp::kRkTX, tcp::kRkTY);
+        const dim3 grid((s->nx + tcp::kRkTX - 1) / tcp::kRkTX, (s->ny + tcp::kRkTY - 1) / tcp::kRkTY, (s->nz + tcp::kRkCZ - 1) / tcp::kRkCZ);
+        if (s->walls) tcp::rk_stage_march_kernel<real, true><<<grid, block, 0, s->stream>>>(R);
+        else tcp::rk_stage_march_kernel<real, false><<<grid, block, 0, s->stream>>>(R);
+        return;
+    }
     const unsigned grid = grid_for(s->N);
     if (s->walls) tcp::rk_stage_kernel<real, true><<<grid, tcp::kBlock, 0, s->stream>>>(R);
     else tcp::rk_stage_kernel<real, false><<<grid, tcp::kBlock, 0, s->stream>>>(R);

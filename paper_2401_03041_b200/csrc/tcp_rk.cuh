@@ -1,0 +1,155 @@
+// rk_stage_march_kernel: one Runge-Kutta stage of eq. 4 (eqs. 25-26) as a z-marching stencil kernel.
+//
+// The stage needs the 27-point gradient and Laplacian of the stage field Y and the gradient of
+// phi^{n+1} and moves only 7-9 values per cell, so 54 global (or shared) loads per cell would make it
+// load-issue bound far above its HBM floor (measured: 1.8 ms per stage at 400^3 against 0.55 ms).
+// Here a block owns a TX x TY tile in (x, y) and walks a chunk of z planes: each plane's tile + halo
+// is staged once in shared memory (ghost rules applied by the loader), every thread reduces its 3 x 3
+// in-plane neighbourhood to S_xS_y, D_xS_y, S_xD_y (9 shared loads per field and plane) and keeps
+// those for three consecutive planes in registers; the z-direction of the tensor-product stencil
+// (reading S3) then closes on registers.  Same arithmetic, in the same order, as stencil27.
+#pragma once
+#include "tcp_step.cuh"
+
+namespace tcp {
+
+constexpr int kRkTX = 32, kRkTY = 8, kRkCZ = 32;
+// 92 registers without a bound = 2 blocks of 256 per SM and 61 % of cycles without an eligible warp (ncu);
+// 3 blocks cost 48 B of spills
+#ifndef TCP_RK_MINB
+#define TCP_RK_MINB 3
+#endif
+
+template <typename real>
+struct Plane3 {          // in-plane reductions of one field on one z plane
+    real S, Dx, Dy, c;
+};
+
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(kRkTX * kRkTY, TCP_RK_MINB) rk_stage_march_kernel(const RkArgs<real> R) {
+    const StepArgs<real>& A = R.S;
+    constexpr int TX = kRkTX, TY = kRkTY, PX = TX + 2, PY = TY + 2, PE = PX * PY;
+    __shared__ real tileY[2][PE], tileP[2][PE];
+    const int tid = threadIdx.y * TX + threadIdx.x;
+    const int bx0 = blockIdx.x * TX, by0 = blockIdx.y * TY, z0 = blockIdx.z * kRkCZ;
+    const int nzc = min(kRkCZ, A.nz - z0);
+    const int x = bx0 + threadIdx.x, y = by0 + threadIdx.y;
+    const bool inside = x < A.nx && y < A.ny;
+    const long long N = A.ncell;
+    const int sy = A.nx, sz = A.nx * A.ny;
+    const bool wx = WALLS && A.wall[0], wy = WALLS && A.wall[1], wz = WALLS && A.wall[2];
+
+    // loader.  Thread t owns halo-tile elements e = t and t + TX*TY (if < PE); their in-plane source
+    // coordinates and wall flags do not depend on z, so they are resolved once.
+    constexpr int NE = (PE + TX * TY - 1) / (TX * TY);
+    int e_idx2d[NE], e_tang_x[NE], e_tang_y[NE], e_fx[NE], e_fy[NE];
+    bool e_on[NE];
+#pragma unroll
+    for (int i = 0; i < NE; ++i) {
+        const int e = tid + i * TX * TY;
+        e_on[i] = e < PE;
+        const int ty = e / PX, tx = e - ty * PX;
+        int X = bx0 + tx - 1, Y = by0 + ty - 1, fx = -1, fy = -1;
+        if (X < 0) { if (wx) { fx = 0; X = 0; } else X += A.nx; }
+        else if (X >= A.nx) { if (X == A.nx) { if (wx) { fx = 1; X = A.nx - 1; } else X = 0; } else X = A.nx - 1; }
+        if (Y < 0) { if (wy) { fy = 0; Y = 0; } else Y += A.ny; }
+        else if (Y >= A.ny) { if (Y == A.ny) { if (wy) { fy = 1; Y = A.ny - 1; } else Y = 0; } else Y = A.ny - 1; }
+        if (X < 0) X = 0;          // nx == 1 corner of an overhanging tile
+        if (Y < 0) Y = 0;
+        e_idx2d[i] = X + sy * Y; e_fx[i] = fx; e_fy[i] = fy; e_tang_x[i] = X; e_tang_y[i] = Y;
+    }
+    real pfY[NE], pfP[NE];          // prefetched plane (in flight while the previous one is consumed)
+    auto fetch_plane = [&](int zreq) {
+        int fz = -1, Z = zreq;
+        if (Z < 0) { if (wz) { fz = 0; Z = 0; } else Z += A.nz; }
+        else if (Z >= A.nz) { if (wz) { fz = 1; Z = A.nz - 1; } else Z -= A.nz; }
+#pragma unroll
+        for (int i = 0; i < NE; ++i) {
+            if (!e_on[i]) continue;
+            const int idx = e_idx2d[i] + sz * Z;
+            real vy = __ldg(R.Y + idx);
+            pfP[i] = __ldg(A.phi_in + idx);
+            if (WALLS) {   // Dirichlet ghost 2 T_w - Y(mirror); first crossed axis in x, y, z order (S9, S17)
+                if (e_fx[i] >= 0) vy = real(2) * A.wallT[0][e_fx[i]][Z * A.ny + e_tang_y[i]] - vy;
+                else if (e_fy[i] >= 0) vy = real(2) * A.wallT[1][e_fy[i]][Z * A.nx + e_tang_x[i]] - vy;
+                else if (fz >= 0) vy = real(2) * A.wallT[2][fz][e_tang_y[i] * A.nx + e_tang_x[i]] - vy;
+            }
+            pfY[i] = vy;
+        }
+    };
+    auto store_plane = [&](int buf) {
+#pragma unroll
+        for (int i = 0; i < NE; ++i)
+            if (e_on[i]) { tileY[buf][tid + i * TX * TY] = pfY[i]; tileP[buf][tid + i * TX * TY] = pfP[i]; }
+    };
+    const real c16 = real(1.0 / 6.0), c23 = real(2.0 / 3.0), half = real(0.5);
+    auto reduce_plane = [&](const real* t) {
+        Plane3<real> P;
+        real sx[3], dxv[3];
+#pragma unroll
+        for (int oy = 0; oy < 3; ++oy) {
+            const real* row = t + (threadIdx.y + oy) * PX + threadIdx.x;
+            const real m = row[0], c = row[1], p = row[2];
+            if (oy == 1) P.c = c;
+            sx[oy] = (m + p) * c16 + c * c23;
+            dxv[oy] = (p - m) * half;
+        }
+        P.S = (sx[0] + sx[2]) * c16 + sx[1] * c23;
+        P.Dy = (sx[2] - sx[0]) * half;
+        P.Dx = (dxv[0] + dxv[2]) * c16 + dxv[1] * c23;
+        return P;
+    };
+
+    // plane p_j = z0 - 1 + j lives in buffer j & 1
+    Plane3<real> Ym, Yc, Yp, Pm, Pc, Pp;   // planes z-1, z, z+1 of Y and phi
+    fetch_plane(z0 - 1); store_plane(0);
+    fetch_plane(z0); store_plane(1);
+    fetch_plane(z0 + 1);                   // stays in registers until iteration 0 stores it
+    __syncthreads();
+    Ym = reduce_plane(tileY[0]); Pm = reduce_plane(tileP[0]);
+    Yc = reduce_plane(tileY[1]); Pc = reduce_plane(tileP[1]);
+    __syncthreads();                       // buffer 0 may now be overwritten
+    for (int k = 0; k < nzc; ++k) {
+        const int buf = k & 1;
+        // cell data of plane z0 + k, requested before the barrier so that its latency hides behind it
+        const int cell = x + sy * y + sz * (z0 + k);
+        real u[3] = {real(0), real(0), real(0)}, Tn = real(0), acc = real(0), qT = real(0);
+        if (inside) {
+            u[0] = A.u[cell]; u[1] = A.u[N + cell]; u[2] = A.u[2 * N + cell];
+            Tn = R.Tn[cell];
+            if (R.mode >= 2) acc = R.acc_in[cell];
+            if (A.q_src) qT = A.q_src[cell];
+        }
+        store_plane(buf);                          // plane z0 + k + 1
+        if (k + 1 < nzc) fetch_plane(z0 + k + 2);  // next one: its latency hides behind this iteration
+        __syncthreads();
+        Yp = reduce_plane(tileY[buf]); Pp = reduce_plane(tileP[buf]);
+        if (inside) {
+            real gY[3], G[3];
+            gY[0] = (Ym.Dx + Yp.Dx) * c16 + Yc.Dx * c23;
+            gY[1] = (Ym.Dy + Yp.Dy) * c16 + Yc.Dy * c23;
+            gY[2] = (Yp.S - Ym.S) * half;
+            const real lapY = real(6) * (((Ym.S + Yp.S) * c16 + Yc.S * c23) - Yc.c);
+            G[0] = (Pm.Dx + Pp.Dx) * c16 + Pc.Dx * c23;
+            G[1] = (Pm.Dy + Pp.Dy) * c16 + Pc.Dy * c23;
+            G[2] = (Pp.S - Pm.S) * half;
+            const real phi_c = Pc.c;
+            const real kap = A.kappa_L + phi_c * A.dkappa;
+            const real rcp = (A.rho_L + phi_c * A.drho) * (A.cp_L + phi_c * A.dcp);
+            const real adv = u[0] * gY[0] + u[1] * gY[1] + u[2] * gY[2];
+            const real dk = A.dkappa * (G[0] * gY[0] + G[1] * gY[1] + G[2] * gY[2]);
+            const real rhs = -adv + (dk + kap * lapY) / rcp + qT;
+            if (R.mode == 3) {
+                R.out[cell] = acc + R.c_acc * rhs;
+            } else {
+                R.out[cell] = Tn + R.c_out * rhs;
+                if (R.mode == 1) R.acc_out[cell] = Tn + R.c_acc * rhs;
+                if (R.mode == 2) R.acc_out[cell] = acc + R.c_acc * rhs;
+            }
+        }
+        Ym = Yc; Yc = Yp; Pm = Pc; Pc = Pp;
+        // no second barrier: iteration k+1 overwrites the OTHER buffer, last read before this iteration's barrier
+    }
+}
+
+}  // namespace tcp

@@ -11,7 +11,9 @@
 #include <cstdlib>
 
 #include "tcp_rk.cuh"
+#ifdef TCP_EXPERIMENTAL_ROWS
 #include "tcp_rows.cuh"
+#endif
 
 namespace {
 
@@ -69,8 +71,6 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
     if (!(p->kappa_H > 0) || !(p->kappa_L > 0) || !(p->cp_H > 0) || !(p->cp_L > 0)) return fail(TCP_EINVAL, "kappa and cp must be > 0");
     if (!(p->eps_normal >= 0)) return fail(TCP_EINVAL, "eps_normal must be >= 0");
     if (p->streaming == TCP_STREAM_AA) return fail(TCP_EUNSUPPORTED, "AA in-place streaming is not built yet");
-    if (!p->high_rate_equals_shear && p->s_high != 1.0)
-        return fail(TCP_EUNSUPPORTED, "s_high != 1 needs the general central-moment transform (not built yet)");
     return TCP_OK;
 }
 
@@ -149,6 +149,7 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     A.cp_L = (real)P.cp_L; A.dcp = (real)(P.cp_H - P.cp_L);
     for (int a = 0; a < 3; ++a) A.grav[a] = (real)P.gravity[a];
     A.s_bulk = (real)P.s_bulk;
+    A.s_high = (real)P.s_high;
     // S8: eps keeps n = grad phi / |grad phi| finite where grad phi vanishes.  In fp32 a gradient
     // below ~1e-6 is round-off of phi ~ 1, and a round-off-directed sharpening flux makes phi = 0 / 1
     // unstable to noise (measured: 1e-4 error after 100 steps next to a wall), so eps is floored there.
@@ -158,26 +159,27 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
 
 unsigned grid_for(size_t n) { return (unsigned)((n + tcp::kBlock - 1) / tcp::kBlock); }
 
-template <typename real, bool WALLS, bool BGK>
+// register-staged kernel: kept for A/B runs (TCP_KERNEL=flat), fast central-moment mode only
+template <typename real, bool WALLS>
 void launch_fused(const tcp_sim* s, const tcp::StepArgs<real>& A) {
     const unsigned grid = grid_for(s->N);
     switch (thermal_q(s->P.thermal)) {
-    case 7: tcp::fused_step_kernel<real, 7, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 15: tcp::fused_step_kernel<real, 15, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 19: tcp::fused_step_kernel<real, 19, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 27: tcp::fused_step_kernel<real, 27, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    default: tcp::fused_step_kernel<real, 0, WALLS, BGK><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 7: tcp::fused_step_kernel<real, 7, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 15: tcp::fused_step_kernel<real, 15, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 19: tcp::fused_step_kernel<real, 19, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    case 27: tcp::fused_step_kernel<real, 27, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    default: tcp::fused_step_kernel<real, 0, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
     }
 }
 
-template <typename real, bool WALLS, bool BGK>
+template <typename real, bool WALLS, int MODE>
 int launch_async(const tcp_sim* s, const tcp::StepArgs<real>& A) {
     const unsigned grid = grid_for(s->N);
     const int QT = thermal_q(s->P.thermal);
     const size_t smem = (size_t)(54 + QT) * tcp::kBlock * sizeof(real);
 #define TCP_ASYNC_LAUNCH(Q)                                                                               \
     do {                                                                                                  \
-        auto kern = tcp::fused_step_async_kernel<real, Q, WALLS, BGK>;                                    \
+        auto kern = tcp::fused_step_async_kernel<real, Q, WALLS, MODE>;                                    \
         CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));           \
         kern<<<grid, tcp::kBlock, smem, s->stream>>>(A);                                                  \
     } while (0)
@@ -206,6 +208,7 @@ void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
     else tcp::rk_stage_kernel<real, false><<<grid, tcp::kBlock, 0, s->stream>>>(R);
 }
 
+#ifdef TCP_EXPERIMENTAL_ROWS
 template <typename real, bool WALLS>
 int launch_rows(const tcp_sim* s, const tcp::StepArgs<real>& A) {
     const dim3 grid((unsigned)((s->nx + s->rows_L - 1) / s->rows_L), (unsigned)s->ny, (unsigned)s->nz);
@@ -227,21 +230,27 @@ int launch_rows(const tcp_sim* s, const tcp::StepArgs<real>& A) {
     return TCP_OK;
 }
 
+#endif
+
 // one time step: Algorithm 1 (thermal LB, one fused kernel) or Algorithm 2 (fused phase+hydro
 // kernel, then the Runge-Kutta stages)
 template <typename real>
 int step_once(tcp_sim* s) {
     tcp::StepArgs<real> A = make_args<real>(s);
-    const bool bgk = s->P.high_rate_equals_shear != 0;
-    if (s->use_async) {
-        int rc = s->walls ? (bgk ? launch_async<real, true, true>(s, A) : launch_async<real, true, false>(s, A))
-                          : (bgk ? launch_async<real, false, true>(s, A) : launch_async<real, false, false>(s, A));
+    // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
+    const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
+    if (s->use_async || mode != 0) {
+        int rc;
+        if (s->walls) rc = mode == 0 ? launch_async<real, true, 0>(s, A) : (mode == 1 ? launch_async<real, true, 1>(s, A) : launch_async<real, true, 2>(s, A));
+        else          rc = mode == 0 ? launch_async<real, false, 0>(s, A) : (mode == 1 ? launch_async<real, false, 1>(s, A) : launch_async<real, false, 2>(s, A));
         if (rc) return rc;
+#ifdef TCP_EXPERIMENTAL_ROWS
     } else if (s->use_rows) {
         int rc = s->walls ? launch_rows<real, true>(s, A) : launch_rows<real, false>(s, A);
         if (rc) return rc;
-    } else if (s->walls) { if (bgk) launch_fused<real, true, true>(s, A); else launch_fused<real, true, false>(s, A); }
-    else                 { if (bgk) launch_fused<real, false, true>(s, A); else launch_fused<real, false, false>(s, A); }
+#endif
+    } else if (s->walls) launch_fused<real, true>(s, A);
+    else launch_fused<real, false>(s, A);
     s->launches++;
     const int th = s->P.thermal;
     if (th == TCP_THERMAL_RK2 || th == TCP_THERMAL_RK4) {
@@ -362,13 +371,13 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
         // TCP_KERNEL=flat / rows overrides (tuning and A/B tests); TCP_ROWS_L sets the segment length.
         const int es = p->precision == TCP_F64 ? 8 : 4, AH = 16 / es;
         const char* force = std::getenv("TCP_KERNEL");
-        s->use_rows = p->bc[0] == TCP_BC_PERIODIC && nx % AH == 0 && !p->high_rate_equals_shear;
+        s->use_rows = p->bc[0] == TCP_BC_PERIODIC && nx % AH == 0 && !p->high_rate_equals_shear && p->s_high == 1.0;
         s->bz = 1;   // measured at 400^3: slabs of 8 / 16 / 32 planes are 2-3 % SLOWER than plain z order (profiles/r01_notes.md)
         if (const char* b = std::getenv("TCP_BZ")) { int v = std::atoi(b); if (v >= 1) s->bz = v < nz ? v : nz; }
         // default: the cp.async staged kernel; TCP_KERNEL=flat (register-staged) / rows (TMA bulk rows) for A/B runs
         s->use_async = !force || std::strcmp(force, "async") == 0;
         if (!force || std::strcmp(force, "rows") != 0) s->use_rows = false;
-        int cap = tcp::kRowsMaxThreads;
+        int cap = 128;
         if (const char* l = std::getenv("TCP_ROWS_L")) { int v = std::atoi(l); if (v >= AH && v <= cap) cap = v; }
         const int nseg = (nx + cap - 1) / cap;
         int L = (nx + nseg - 1) / nseg;

@@ -28,7 +28,7 @@ struct StepArgs {
     real sigma_ref, sigma_T, T_ref;  // eq. 9
     real kappa_L, dkappa, cp_L, dcp; // eqs. 23-24 (reading G5)
     real grav[3];                    // eq. 7
-    real s_bulk, eps;
+    real s_bulk, s_high, eps;
 };
 
 // ---------------------------------------------------------------------------------------------

@@ -83,7 +83,7 @@ constexpr int kRowsMaxThreads = TCP_ROWS_MAXT;
 
 template <typename real, int QT, bool WALLS>
 __global__ void __launch_bounds__(TCP_ROWS_MAXT, TCP_ROWS_MINB) fused_step_rows_kernel(const StepArgs<real> A_, int Lseg) {
-    constexpr bool BGK = false;
+    constexpr int MODE = 0;
     constexpr int AH = RowGeom<real>::A;
     const StepArgs<real>& A = A_;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(TCP_ROWS_MAXT, TCP_ROWS_MINB) fused_step_rows_
         real h[27];
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = staged(q, q);
-        phi_new = collide_phase<real, BGK>(A, h, G, phi_c, u);
+        phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
         if (active) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = h[q];
@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(TCP_ROWS_MAXT, TCP_ROWS_MINB) fused_step_rows_
         real g[27];
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = staged(27 + q, q);
-        collide_hydro<real, BGK>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+        collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
         if (active) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(TCP_ROWS_MAXT, TCP_ROWS_MINB) fused_step_rows_
                 f[k] = rows[(size_t)(54 + k) * P + t + AH - cx];
         });
         const real qT = A.q_src ? A.q_src[cell] : real(0);
-        const real Tn = collide_thermal<real, QT, BGK>(A, f, phi_new, u, qT);
+        const real Tn = collide_thermal<real, QT, MODE>(A, f, phi_new, u, qT);
         if (active) {
             static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
             A.T_out[cell] = Tn;

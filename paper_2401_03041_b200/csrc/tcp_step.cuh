@@ -38,10 +38,42 @@ __device__ __forceinline__ void conserve_zeroth27(real a[27], double s) {
     }
 }
 
+// In-place central-moment transform of a D3Q27 population set indexed 9 c_z + 3 c_y + c_x (+13):
+// forward: populations -> kappa_{abc} stored at 9c + 3b + a; inverse: back.  Three sweeps of the
+// 1-D transform on {-1, 0, 1}:  k0 = sum p, k1 = sum (c - u) p, k2 = sum (c - u)^2 p.
+template <typename real, bool FORWARD>
+__device__ __forceinline__ void central_transform27(real X[27], const real u[3]) {
+#pragma unroll
+    for (int pass = 0; pass < 3; ++pass) {
+        const int axis = FORWARD ? pass : 2 - pass;
+        const int stride = axis == 0 ? 1 : (axis == 1 ? 3 : 9);
+        const real ua = u[axis], uu = ua * ua;
+#pragma unroll
+        for (int j = 0; j < 9; ++j) {
+            // base index of the j-th line along `axis`
+            const int base = axis == 0 ? 3 * j : (axis == 1 ? (j / 3) * 9 + (j % 3) : j);
+            real& e0 = X[base]; real& e1 = X[base + stride]; real& e2 = X[base + 2 * stride];
+            if (FORWARD) {
+                const real m = e0, c = e1, p = e2;
+                const real m0 = (m + p) + c, m1 = p - m, m2 = p + m;
+                e0 = m0;
+                e1 = m1 - ua * m0;
+                e2 = m2 - real(2) * ua * m1 + uu * m0;
+            } else {
+                const real k0 = e0, k1 = e1, k2 = e2;
+                const real m1 = k1 + ua * k0, m2 = k2 + real(2) * ua * k1 + uu * k0;
+                e0 = real(0.5) * (m2 - m1);
+                e1 = k0 - m2;
+                e2 = real(0.5) * (m2 + m1);
+            }
+        }
+    }
+}
+
 // ---- phase-field LB on one cell: eqs. 10-15 ---------------------------------------------------
 // h = pulled populations; G = grad phi^n, phi_c = phi^n (interface force from the stored phi,
 // reading S10); un = u^n.  Writes h~ and phi' = sum h (eq. 13).
-template <typename real, bool BGK>
+template <typename real, int MODE>
 __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27], const real G[3], real phi_c, const real un[3]) {
     const Mom2<real> M = moments27<real, false>(h);
     double phin_exact = 0.0;
@@ -52,7 +84,7 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
     const real mag = real(4.0 / 3.0) * phi_c * (real(1) - phi_c) / A.xi * inv;
     real a[3] = {mag * G[0], mag * G[1], mag * G[2]};
     const real w = A.w_phi;
-    if (BGK) {   // a~ = (1-w) a + w [a_eq + F(a (2-w)/w)/2]
+    if (MODE == 1) {   // a~ = (1-w) a + w [a_eq + F(a (2-w)/w)/2]
         const real sc = (real(2) - w) / w;
         a[0] *= sc; a[1] *= sc; a[2] *= sc;
     }
@@ -62,7 +94,7 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
     const real A0 = phin - real(1.5) * (un[0] * b[0] + un[1] * b[1] + un[2] * b[2]);
     real out[27];
     equilibrium_plus_half_force27<real>(A0, un, v, b, out);
-    if (BGK) {
+    if (MODE == 1) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = (real(1) - w) * h[q] + w * out[q];
     } else {
@@ -83,7 +115,7 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
 
 // ---- hydrodynamic LB on one cell: eqs. 16-22, forces of eqs. 7-9 -------------------------------
 // g = pulled populations; phi_c, G, lapPhi from phi^n (S16); T_c, Th = grad T^n.  Writes g~, u^{n+1}.
-template <typename real, bool BGK>
+template <typename real, int MODE>
 __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27], real phi_c, const real G[3], real lapPhi,
                                               real T_c, const real Th[3], real u[3]) {
     const Mom2<real> M = moments27<real, true>(g);
@@ -124,7 +156,7 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
         u[al] = j[al] + F[al] * i2r;                        // u^{n+1} (S6)
         a[al] = real(2) * F[al] * i2r;                      // Guo vector F / rho
     }
-    if (BGK) {
+    if (MODE == 1) {
         const real sc = (real(2) - om) / om;
         a[0] *= sc; a[1] *= sc; a[2] *= sc;
     }
@@ -134,9 +166,35 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
     const real A0 = ps - real(1.5) * (u[0] * b[0] + u[1] * b[1] + u[2] * b[2]);
     real out[27];
     equilibrium_plus_half_force27<real>(A0, u, v, b, out);
-    if (BGK) {
+    if (MODE == 1) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = (real(1) - om) * g[q] + om * out[q];
+    } else if (MODE == 2) {
+        // general rates (s_high != 1): g~ = E + K^-1 (I - S) K X,  X = (g - g_eq) + F/2 = g - E(-a)
+        // (I - S vanishes on orders 0 and 1).  K is applied as three sweeps of the 1-D central-moment
+        // transform (x, y, z), its inverse as the reverse sweeps.
+        real X[27];
+        {
+            real bm[3], vm[3];
+#pragma unroll
+            for (int al = 0; al < 3; ++al) { bm[al] = u[al] - a[al]; vm[al] = u[al] - real(0.5) * a[al]; }
+            equilibrium_plus_half_force27<real>(ps - real(1.5) * (u[0] * bm[0] + u[1] * bm[1] + u[2] * bm[2]), u, vm, bm, X);
+#pragma unroll
+            for (int q = 0; q < 27; ++q) X[q] = g[q] - X[q];
+        }
+        central_transform27<real, true>(X, u);
+        const real k2 = real(1) - om, k3 = real(1) - A.s_high;
+        const real tr3 = (X[2] + X[6] + X[18]) * real(1.0 / 3.0), kb = (real(1) - A.s_bulk) * tr3;
+#pragma unroll
+        for (int q = 0; q < 27; ++q) {
+            const int order = (q % 3) + (q / 3) % 3 + q / 9;
+            if (order <= 1) X[q] = real(0);
+            else if (order == 2) X[q] = (q == 2 || q == 6 || q == 18) ? k2 * (X[q] - tr3) + kb : k2 * X[q];
+            else X[q] = k3 * X[q];
+        }
+        central_transform27<real, false>(X, u);
+#pragma unroll
+        for (int q = 0; q < 27; ++q) g[q] = out[q] + X[q];
     } else {
         // second-order central moments of g - g_eq: deviatoric part relaxes with omega, trace with
         // s_bulk, everything else with 1 (reading S2); Guo populations have none
@@ -160,7 +218,7 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
 }
 
 // ---- thermal LB on one cell: eqs. 27-29 (rho c_p = 1 on this path, S11) ------------------------
-template <typename real, int Q, bool BGK>
+template <typename real, int Q, int MODE>
 __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[Q], real phi_new, const real u[3], real qT) {
     real Tn = real(0), j[3] = {real(0), real(0), real(0)};
     double Tn_exact = 0.0;
@@ -177,7 +235,7 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
     const real w = real(1) / (real(0.5) + real(3) * kap);    // eq. 29 read as a rate (G4)
     real out[Q];
     thermal_equilibrium<real, Q>(Tn, u, out);
-    if (BGK) {
+    if (MODE == 1) {
         static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; out[k] = (real(1) - w) * f[k] + w * out[k]; });
     } else {
         const real k1 = real(1) - w;
@@ -203,7 +261,7 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
 }
 
 // ---------------------------------------------------------------------------------------------
-template <typename real, int QT, bool WALLS, bool BGK>
+template <typename real, int QT, bool WALLS, int MODE>
 __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const StepArgs<real> A) {
     const int gtid = blockIdx.x * kBlock + threadIdx.x;
     if (gtid >= A.ncell) return;
@@ -221,7 +279,7 @@ __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const Step
     {
         real h[27];
         pull27<real, WALLS>(A, nb, A.h_in, h);
-        phi_new = collide_phase<real, BGK>(A, h, G, phi_c, u);
+        phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
 #pragma unroll
         for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = h[q];
         A.phi_out[cell] = phi_new;
@@ -229,7 +287,7 @@ __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const Step
     {
         real g[27];
         pull27<real, WALLS>(A, nb, A.g_in, g);
-        collide_hydro<real, BGK>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+        collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
 #pragma unroll
         for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
         A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
@@ -238,7 +296,7 @@ __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const Step
         real f[QT];
         pull_thermal<real, QT, WALLS>(A, nb, A.f_in, f);
         const real qT = A.q_src ? A.q_src[cell] : real(0);
-        const real Tn = collide_thermal<real, QT, BGK>(A, f, phi_new, u, qT);
+        const real Tn = collide_thermal<real, QT, MODE>(A, f, phi_new, u, qT);
         static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
         A.T_out[cell] = Tn;
     }
@@ -269,7 +327,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 template <typename real, int QT>
 constexpr int async_min_blocks() { return (sizeof(real) == 8 && QT >= 15) ? 2 : TCP_MINB; }
 
-template <typename real, int QT, bool WALLS, bool BGK>
+template <typename real, int QT, bool WALLS, int MODE>
 __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_step_async_kernel(const StepArgs<real> A) {
     extern __shared__ __align__(16) unsigned char smem_raw_async[];
     real* stage = reinterpret_cast<real*>(smem_raw_async);     // [54 + QT][kBlock]
@@ -318,7 +376,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         real h[27];
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = stage[q * kBlock + tid];
-        phi_new = collide_phase<real, BGK>(A, h, G, phi_c, u);
+        phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
         if (active) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = h[q];
@@ -330,7 +388,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         real g[27];
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = stage[(27 + q) * kBlock + tid];
-        collide_hydro<real, BGK>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+        collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
         if (active) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
@@ -351,7 +409,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
                 f[k] = v;
         });
         const real qT = A.q_src ? A.q_src[cell] : real(0);
-        const real Tn = collide_thermal<real, QT, BGK>(A, f, phi_new, u, qT);
+        const real Tn = collide_thermal<real, QT, MODE>(A, f, phi_new, u, qT);
         if (active) {
             static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
             A.T_out[cell] = Tn;

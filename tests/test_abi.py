@@ -52,7 +52,7 @@ def test_workspace_bytes_accounting():
 @pytest.mark.parametrize("bad, code", [
     (dict(M=0.0), tcp.TCP_EINVAL), (dict(xi=-1.0), tcp.TCP_EINVAL), (dict(tau_H=-0.5), tcp.TCP_EINVAL),
     (dict(rho_L=0.0), tcp.TCP_EINVAL), (dict(kappa_H=0.0), tcp.TCP_EINVAL),
-    (dict(streaming="aa"), tcp.TCP_EUNSUPPORTED), (dict(s_high=1.2), tcp.TCP_EUNSUPPORTED),
+    (dict(streaming="aa"), tcp.TCP_EUNSUPPORTED),
 ])
 def test_parameter_validation(bad, code):
     with pytest.raises(tcp.TcpError) as e:
@@ -68,7 +68,8 @@ def test_extent_validation():
             tcp.tcp_workspace_bytes(*dims, p)
         assert e.value.code == tcp.TCP_EINVAL
     assert tcp.tcp_workspace_bytes(1, 2, 1, p) > 0
-    # s_high is ignored in BGK mode
+    # any s_high is accepted (general central-moment mode), also together with BGK mode (where it is ignored)
+    assert tcp.tcp_workspace_bytes(4, 4, 4, tcp.make_params(dict(s_high=1.3))) > 0
     assert tcp.tcp_workspace_bytes(4, 4, 4, tcp.make_params(dict(s_high=1.3, high_rate_equals_shear=1))) > 0
 
 

@@ -88,6 +88,17 @@ def test_bgk_mode_and_bulk_rate():
     _check(wl, extra=dict(high_rate_equals_shear=1))
 
 
+@pytest.mark.parametrize("rates", [dict(s_high=1.3), dict(s_high=0.7, s_bulk=1.5), dict(s_high=1.5, s_bulk=0.8)])
+def test_general_central_moment_rates(rates):
+    """s_high != 1 (rate of the central moments of order >= 3 of the hydrodynamic lattice, reading S2):
+    the kernels switch from the closed form to the full central-moment transform."""
+    wl = W.perf_box(20, thermal="lb_d3q7", ny=18, nz=14, r_min=3.0, r_max=4.0, seed=4)
+    wl.u = torch.from_numpy(0.02 * np.random.default_rng(1).standard_normal((3, 14, 18, 20)))
+    _check(wl, extra=rates)
+    wl = W.layered_channel(nx=24, ny=16, nz=2, thermal="rk2", rho_upper=3.0)
+    _check(wl, extra=rates)
+
+
 def test_heat_source_and_gravity():
     """q_T of eqs. 4 / 27 (a Gaussian spot, eq. 37 shape) and a body force (eq. 7)."""
     for thermal in ("lb_d3q7", "rk2"):

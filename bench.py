@@ -174,7 +174,7 @@ def run_ours(args):
     tdt = torch.float64 if prec == "f64" else torch.float32
     wl = W.perf_box(n, thermal=thermal, device="cuda", seed=20240103 + n + rank)
     N = wl.cells
-    params = dict(wl.params, precision=prec)
+    params = dict(wl.params, precision=prec, streaming=args.streaming)
     sim = tcp.Simulation(n, n, n, params)
     phi_d, T_d = wl.phi.to(tdt).contiguous(), wl.T.to(tdt).contiguous()
     sim.init_fields(phi_d, None, T_d)
@@ -256,7 +256,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": prec, "data": "synthetic",
-            "config": {"workload": f"perf_box {n}^3 periodic (BASELINE configs[4]), hydro D3Q27 CM, phase D3Q27, thermal {thermal}",
+            "config": {"workload": f"perf_box {n}^3 periodic (BASELINE configs[4]), hydro D3Q27 CM, phase D3Q27, thermal {thermal}, streaming {args.streaming}",
                        "cells_per_gpu": N, "parallelism": "replicas" if world > 1 else "single GPU",
                        "l2": f"working set {step_bytes / 1e9:.1f} GB per step >> 126 MB L2, no flush needed",
                        "notes": wl.notes},
@@ -281,7 +281,7 @@ def run_sweep(args):
         tdt = torch.float64 if prec == "f64" else torch.float32
         for thermal in ("lb_d3q7", "lb_d3q15", "lb_d3q19", "lb_d3q27", "rk2", "rk4"):
             wl = W.perf_box(n, thermal=thermal, device="cuda")
-            sim = tcp.Simulation(n, n, n, dict(wl.params, precision=prec))
+            sim = tcp.Simulation(n, n, n, dict(wl.params, precision=prec, streaming=args.streaming))
             sim.init_fields(wl.phi.to(tdt).contiguous(), None, wl.T.to(tdt).contiguous())
             sim.step(max(args.warmup, 3))
             times = []
@@ -293,7 +293,7 @@ def run_sweep(args):
             sim.close()
             bpc = step_values_per_cell(thermal) * es
             gbs = bpc * n ** 3 / (ms * 1e-3) / 1e9
-            print(json.dumps({"sweep": True, "size": n, "dtype": prec, "thermal": thermal, "ms_per_step": ms,
+            print(json.dumps({"sweep": True, "size": n, "dtype": prec, "thermal": thermal, "streaming": args.streaming, "ms_per_step": ms,
                               "mlups": n ** 3 / (ms * 1e-3) / 1e6, "step_bytes_per_cell": bpc, "gbs": gbs,
                               "frac_of_measured_peak": gbs / peak, "finite": finite}), flush=True)
             del sim, wl
@@ -308,6 +308,7 @@ def main():
     ap.add_argument("--size", type=int, default=400)
     ap.add_argument("--thermal", default="lb_d3q7", choices=sorted(QT))
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--streaming", default="two_grid", choices=["two_grid", "aa"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-size", type=int, default=40)
     ap.add_argument("--no-e2e", action="store_true")

@@ -36,7 +36,7 @@ enum { TCP_F64 = 0, TCP_F32 = 1 };
 enum { TCP_THERMAL_LB_D3Q7 = 0, TCP_THERMAL_LB_D3Q15, TCP_THERMAL_LB_D3Q19, TCP_THERMAL_LB_D3Q27,
        TCP_THERMAL_RK2, TCP_THERMAL_RK4 };
 enum { TCP_BC_PERIODIC = 0, TCP_BC_WALLS = 1 };
-enum { TCP_STREAM_TWO_GRID = 0, TCP_STREAM_AA = 1 }; /* AA: not built yet -> TCP_EUNSUPPORTED */
+enum { TCP_STREAM_TWO_GRID = 0, TCP_STREAM_AA = 1 }; /* AA: in place, one grid of populations (half the memory) */
 
 /* The paper's problem statement (sections 2.1-2.3).  Fill `struct_size = sizeof(tcp_params)`. */
 typedef struct tcp_params {

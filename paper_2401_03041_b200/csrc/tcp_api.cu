@@ -10,6 +10,7 @@
 #include "../../include/tcp.h"
 #include <cstdlib>
 
+#include "tcp_launch.h"
 #include "tcp_rk.cuh"
 #ifdef TCP_EXPERIMENTAL_ROWS
 #include "tcp_rows.cuh"
@@ -70,7 +71,6 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
     if (!(p->rho_H > 0) || !(p->rho_L > 0)) return fail(TCP_EINVAL, "rho must be > 0");
     if (!(p->kappa_H > 0) || !(p->kappa_L > 0) || !(p->cp_H > 0) || !(p->cp_L > 0)) return fail(TCP_EINVAL, "kappa and cp must be > 0");
     if (!(p->eps_normal >= 0)) return fail(TCP_EINVAL, "eps_normal must be >= 0");
-    if (p->streaming == TCP_STREAM_AA) return fail(TCP_EUNSUPPORTED, "AA in-place streaming is not built yet");
     return TCP_OK;
 }
 
@@ -82,9 +82,10 @@ Layout make_layout(int nx, int ny, int nz, const tcp_params* p) {
     const int QT = thermal_q(p->thermal);
     size_t off = 0;
     auto take = [&](size_t count) { size_t o = off; off = align_up(off + count * es); return o; };
-    for (int b = 0; b < 2; ++b) L.h[b] = take(27 * N);
-    for (int b = 0; b < 2; ++b) L.g[b] = take(27 * N);
-    for (int b = 0; b < 2; ++b) L.f[b] = QT ? take((size_t)QT * N) : 0;
+    const bool aa = p->streaming == TCP_STREAM_AA;      // in-place streaming: one grid of populations
+    for (int b = 0; b < 2; ++b) L.h[b] = (aa && b) ? L.h[0] : take(27 * N);
+    for (int b = 0; b < 2; ++b) L.g[b] = (aa && b) ? L.g[0] : take(27 * N);
+    for (int b = 0; b < 2; ++b) L.f[b] = QT ? ((aa && b) ? L.f[0] : take((size_t)QT * N)) : 0;
     for (int b = 0; b < 2; ++b) L.phi[b] = take(N);
     for (int b = 0; b < 2; ++b) L.T[b] = take(N);
     L.u = take(3 * N);
@@ -114,6 +115,7 @@ struct tcp_sim {
     cudaEvent_t ev0, ev1;
     bool use_async;          // cp.async staged kernel
     int bz;                  // z-slab thickness of the cell visiting order
+    int aa_next;             // AA streaming: type of the next step (1 even, 2 odd); 0 = two-grid
     bool use_rows;           // TMA row-segment kernel eligible (x periodic, nx % (16 B / element) == 0, not BGK)
     int rows_L, rows_threads;
     size_t rows_smem;
@@ -131,6 +133,7 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     const int c = s->cur, o = 1 - s->cur;
     A.nx = s->nx; A.ny = s->ny; A.nz = s->nz; A.ncell = (int)s->N;
     A.bz = s->bz;
+    A.aa = s->aa_next;
     for (int a = 0; a < 3; ++a) A.wall[a] = P.bc[a] == TCP_BC_WALLS;
     A.h_in = ptr<real>(s, s->L.h[c]); A.h_out = ptr<real>(s, s->L.h[o]);
     A.g_in = ptr<real>(s, s->L.g[c]); A.g_out = ptr<real>(s, s->L.g[o]);
@@ -158,41 +161,6 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
 }
 
 unsigned grid_for(size_t n) { return (unsigned)((n + tcp::kBlock - 1) / tcp::kBlock); }
-
-// register-staged kernel: kept for A/B runs (TCP_KERNEL=flat), fast central-moment mode only
-template <typename real, bool WALLS>
-void launch_fused(const tcp_sim* s, const tcp::StepArgs<real>& A) {
-    const unsigned grid = grid_for(s->N);
-    switch (thermal_q(s->P.thermal)) {
-    case 7: tcp::fused_step_kernel<real, 7, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 15: tcp::fused_step_kernel<real, 15, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 19: tcp::fused_step_kernel<real, 19, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 27: tcp::fused_step_kernel<real, 27, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    default: tcp::fused_step_kernel<real, 0, WALLS, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    }
-}
-
-template <typename real, bool WALLS, int MODE>
-int launch_async(const tcp_sim* s, const tcp::StepArgs<real>& A) {
-    const unsigned grid = grid_for(s->N);
-    const int QT = thermal_q(s->P.thermal);
-    const size_t smem = (size_t)(54 + QT) * tcp::kBlock * sizeof(real);
-#define TCP_ASYNC_LAUNCH(Q)                                                                               \
-    do {                                                                                                  \
-        auto kern = tcp::fused_step_async_kernel<real, Q, WALLS, MODE>;                                    \
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));           \
-        kern<<<grid, tcp::kBlock, smem, s->stream>>>(A);                                                  \
-    } while (0)
-    switch (QT) {
-    case 7: TCP_ASYNC_LAUNCH(7); break;
-    case 15: TCP_ASYNC_LAUNCH(15); break;
-    case 19: TCP_ASYNC_LAUNCH(19); break;
-    case 27: TCP_ASYNC_LAUNCH(27); break;
-    default: TCP_ASYNC_LAUNCH(0); break;
-    }
-#undef TCP_ASYNC_LAUNCH
-    return TCP_OK;
-}
 
 template <typename real>
 void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
@@ -239,18 +207,19 @@ int step_once(tcp_sim* s) {
     tcp::StepArgs<real> A = make_args<real>(s);
     // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
     const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
-    if (s->use_async || mode != 0) {
-        int rc;
-        if (s->walls) rc = mode == 0 ? launch_async<real, true, 0>(s, A) : (mode == 1 ? launch_async<real, true, 1>(s, A) : launch_async<real, true, 2>(s, A));
-        else          rc = mode == 0 ? launch_async<real, false, 0>(s, A) : (mode == 1 ? launch_async<real, false, 1>(s, A) : launch_async<real, false, 2>(s, A));
-        if (rc) return rc;
+    {
+        tcp::FusedCfg c;
+        c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
+        c.staged = s->use_async || mode != 0 || c.aa != 0;
+        c.grid = grid_for(s->N);
 #ifdef TCP_EXPERIMENTAL_ROWS
-    } else if (s->use_rows) {
-        int rc = s->walls ? launch_rows<real, true>(s, A) : launch_rows<real, false>(s, A);
-        if (rc) return rc;
+        if (!c.staged && s->use_rows) {
+            int rc = s->walls ? launch_rows<real, true>(s, A) : launch_rows<real, false>(s, A);
+            if (rc) return rc;
+        } else
 #endif
-    } else if (s->walls) launch_fused<real, true>(s, A);
-    else launch_fused<real, false>(s, A);
+        CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+    }
     s->launches++;
     const int th = s->P.thermal;
     if (th == TCP_THERMAL_RK2 || th == TCP_THERMAL_RK4) {
@@ -284,6 +253,7 @@ int step_once(tcp_sim* s) {
         }
     }
     s->cur = 1 - s->cur;
+    if (s->aa_next) s->aa_next = 3 - s->aa_next;
     return TCP_OK;
 }
 
@@ -299,6 +269,7 @@ int init_fields_t(tcp_sim* s, const void* phi, const void* u, const void* T) {
         tcp::fill_kernel<real><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(ptr<real>(s, s->L.T[0]), (long long)N, (real)s->P.T_ref);
         s->launches++;
     }
+    s->aa_next = s->P.streaming == TCP_STREAM_AA ? 1 : 0;   // AA: init stores pushed populations, the first step is an even one
     tcp::StepArgs<real> A = make_args<real>(s);
     A.h_out = ptr<real>(s, s->L.h[0]); A.g_out = ptr<real>(s, s->L.g[0]); A.f_out = ptr<real>(s, s->L.f[0]);
     const unsigned grid = grid_for(N);
@@ -339,9 +310,13 @@ int read_fields_t(tcp_sim* s, void* phi, void* u, void* p, void* T) {
     if (T) CK(cudaMemcpyAsync(T, ptr<real>(s, s->L.T[s->cur]), N * es, cudaMemcpyDefault, s->stream));
     if (p) {
         real* scratch = ptr<real>(s, s->L.phi[1 - s->cur]);   // free between steps
-        tcp::pressure_kernel<real><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(ptr<real>(s, s->L.g[s->cur]), ptr<real>(s, s->L.phi[s->cur]),
-                                                                               scratch, (int)N, (real)s->P.rho_L,
-                                                                               (real)(s->P.rho_H - s->P.rho_L));
+        if (s->aa_next == 1)   // AA, populations in the pushed layout (after init or an odd step)
+            tcp::pressure_pushed_kernel<real><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(make_args<real>(s), ptr<real>(s, s->L.g[0]),
+                                                                                        ptr<real>(s, s->L.phi[s->cur]), scratch);
+        else
+            tcp::pressure_kernel<real><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(ptr<real>(s, s->L.g[s->cur]), ptr<real>(s, s->L.phi[s->cur]),
+                                                                                   scratch, (int)N, (real)s->P.rho_L,
+                                                                                   (real)(s->P.rho_H - s->P.rho_L));
         s->launches++;
         CK(cudaGetLastError());
         CK(cudaMemcpyAsync(p, scratch, N * es, cudaMemcpyDefault, s->stream));
@@ -377,6 +352,7 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
         // default: the cp.async staged kernel; TCP_KERNEL=flat (register-staged) / rows (TMA bulk rows) for A/B runs
         s->use_async = !force || std::strcmp(force, "async") == 0;
         if (!force || std::strcmp(force, "rows") != 0) s->use_rows = false;
+        if (p->streaming == TCP_STREAM_AA) { s->use_async = true; s->use_rows = false; }   // only the staged kernel knows the AA addressing
         int cap = 128;
         if (const char* l = std::getenv("TCP_ROWS_L")) { int v = std::atoi(l); if (v >= AH && v <= cap) cap = v; }
         const int nseg = (nx + cap - 1) / cap;

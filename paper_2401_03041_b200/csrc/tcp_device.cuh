@@ -14,6 +14,7 @@ struct StepArgs {
     int nx, ny, nz;
     int ncell;                       // nx*ny*nz < 2^31
     int bz;                          // z-slab thickness of the visiting order (Nbh::init)
+    int aa;                          // streaming: 0 two-grid pull; AA in place: 1 even step, 2 odd step (tcp_step.cuh)
     int wall[3];                     // 1 = WALLS on that axis
     const real* h_in;  real* h_out;  // [27][N]
     const real* g_in;  real* g_out;  // [27][N]

@@ -1,0 +1,24 @@
+// Launchers of the fused step kernels, one translation unit per precision so that the ~70 template
+// instantiations compile in parallel (paper_2401_03041_b200/build.py).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "tcp_device.cuh"
+
+namespace tcp {
+
+struct FusedCfg {
+    int qt;          // thermal stencil size, 0 on the Runge-Kutta paths
+    bool walls;      // any WALLS axis
+    int mode;        // 0 closed-form central moments, 1 BGK, 2 general rates
+    int aa;          // 0 two-grid; AA in-place streaming: 1 even step, 2 odd step
+    bool staged;     // cp.async staged kernel (default) or the register-staged one (mode 0, two-grid only)
+    unsigned grid;
+};
+
+cudaError_t launch_fused_periodic(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
+cudaError_t launch_fused_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
+cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+
+}  // namespace tcp

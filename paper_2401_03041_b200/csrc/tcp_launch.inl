@@ -1,0 +1,56 @@
+// Included by tcp_fused_f64.cu / tcp_fused_f32.cu with TCP_REAL defined.
+#include "tcp_launch.h"
+#include "tcp_step.cuh"
+
+namespace tcp {
+namespace {
+
+template <typename real, int QT, bool WALLS, int MODE, int AA>
+cudaError_t launch_staged(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
+    const size_t smem = (size_t)(54 + QT) * kBlock * sizeof(real);
+    auto kern = fused_step_async_kernel<real, QT, WALLS, MODE, AA>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<c.grid, kBlock, smem, stream>>>(A);
+    return cudaGetLastError();
+}
+
+template <typename real, int QT, bool WALLS>
+cudaError_t dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
+    if (!c.staged && c.mode == 0 && !c.aa) {
+        fused_step_kernel<real, QT, WALLS, 0><<<c.grid, kBlock, 0, stream>>>(A);
+        return cudaGetLastError();
+    }
+    switch (3 * c.aa + c.mode) {   // c.aa: 0 two-grid, 1 AA even step, 2 AA odd step
+    case 0: return launch_staged<real, QT, WALLS, 0, 0>(c, A, stream);
+    case 1: return launch_staged<real, QT, WALLS, 1, 0>(c, A, stream);
+    case 2: return launch_staged<real, QT, WALLS, 2, 0>(c, A, stream);
+    case 3: return launch_staged<real, QT, WALLS, 0, 1>(c, A, stream);
+    case 4: return launch_staged<real, QT, WALLS, 1, 1>(c, A, stream);
+    case 5: return launch_staged<real, QT, WALLS, 2, 1>(c, A, stream);
+    case 6: return launch_staged<real, QT, WALLS, 0, 2>(c, A, stream);
+    case 7: return launch_staged<real, QT, WALLS, 1, 2>(c, A, stream);
+    default: return launch_staged<real, QT, WALLS, 2, 2>(c, A, stream);
+    }
+}
+
+template <typename real, bool WALLS>
+cudaError_t by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
+    switch (c.qt) {
+    case 7: return dispatch<real, 7, WALLS>(c, A, stream);
+    case 15: return dispatch<real, 15, WALLS>(c, A, stream);
+    case 19: return dispatch<real, 19, WALLS>(c, A, stream);
+    case 27: return dispatch<real, 27, WALLS>(c, A, stream);
+    default: return dispatch<real, 0, WALLS>(c, A, stream);
+    }
+}
+
+}  // namespace
+
+#ifdef TCP_WALLS_ONLY
+cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, true>(c, A, stream); }
+#else
+cudaError_t launch_fused_periodic(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, false>(c, A, stream); }
+#endif
+
+}  // namespace tcp

@@ -327,7 +327,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 template <typename real, int QT>
 constexpr int async_min_blocks() { return (sizeof(real) == 8 && QT >= 15) ? 2 : TCP_MINB; }
 
-template <typename real, int QT, bool WALLS, int MODE>
+template <typename real, int QT, bool WALLS, int MODE, int AA>
 __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_step_async_kernel(const StepArgs<real> A) {
     extern __shared__ __align__(16) unsigned char smem_raw_async[];
     real* stage = reinterpret_cast<real*>(smem_raw_async);     // [54 + QT][kBlock]
@@ -339,28 +339,43 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
     nb.init(A, active ? gtid : A.ncell - 1);                   // tail lanes shadow the last cell, store nothing
     const int cell = nb.idx;
 
-    // issue every pull of this cell (bounce-back links copy the opposite direction of the own cell)
-#pragma unroll
-    for (int q = 0; q < 27; ++q) {
+    // Where the pre-collision population of direction q lives (AA in-place streaming, is a
+    // storage permutation only: every step still sees the streamed populations of its cell):
+    //   two-grid   : plane q at x - c_q            (wall link: plane opp(q) at x)
+    //   AA, even   : plane q at x                  (the odd step / init pushed it there)
+    //   AA, odd    : plane opp(q) at x - c_q       (wall link: plane q at x; the even step swapped in place)
+    // and where the post-collision one goes:
+    //   two-grid   : plane q at x (other grid);  AA even: plane opp(q) at x;
+    //   AA odd     : plane q at x + c_q (wall link: plane opp(q) at x, so that the next even step finds it)
+    constexpr int aa = AA;   // 0 two-grid, 1 AA even step, 2 AA odd step: compile-time (a run-time switch cost 20 %)
+    auto src_of = [&](const real* base, int Q, int k, int q27i) -> const real* {
+        const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
+        if (aa == 1) return base + k * N + cell;
         int face = 0;
-        const bool bb = WALLS && nb.crossed(-cx27(q), -cy27(q), -cz27(q), face) >= 0;
-        cp_async_elem<real>(stage + q * kBlock + tid, bb ? A.h_in + (26 - q) * N + cell : A.h_in + q * N + nb.at(-cx27(q), -cy27(q), -cz27(q)));
-    }
+        const bool bb = WALLS && nb.crossed(-cx, -cy, -cz, face) >= 0;
+        const int plane = (bb != (aa == 2)) ? Q - 1 - k : k;
+        return base + plane * N + (bb ? cell : nb.at(-cx, -cy, -cz));
+    };
+    auto dst_of = [&](real* base, int Q, int k, int q27i, bool& wall_link) -> real* {
+        const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
+        wall_link = false;
+        if (aa == 0) return base + k * N + cell;
+        if (aa == 1) return base + (Q - 1 - k) * N + cell;
+        int face = 0;
+        wall_link = WALLS && nb.crossed(cx, cy, cz, face) >= 0;
+        return wall_link ? base + (Q - 1 - k) * N + cell : base + k * N + nb.at(cx, cy, cz);
+    };
+
+#pragma unroll
+    for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + q * kBlock + tid, src_of(A.h_in, 27, q, q));
     cp_async_commit();
 #pragma unroll
-    for (int q = 0; q < 27; ++q) {
-        int face = 0;
-        const bool bb = WALLS && nb.crossed(-cx27(q), -cy27(q), -cz27(q), face) >= 0;
-        cp_async_elem<real>(stage + (27 + q) * kBlock + tid, bb ? A.g_in + (26 - q) * N + cell : A.g_in + q * N + nb.at(-cx27(q), -cy27(q), -cz27(q)));
-    }
+    for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + (27 + q) * kBlock + tid, src_of(A.g_in, 27, q, q));
     cp_async_commit();
     if constexpr (QT > 0) {
         static_for<0, QT>([&](auto K) {
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
-            int face = 0;
-            const bool bb = WALLS && nb.crossed(-cx27(q), -cy27(q), -cz27(q), face) >= 0;
-            cp_async_elem<real>(stage + (54 + k) * kBlock + tid,
-                                bb ? A.f_in + (QT - 1 - k) * N + cell : A.f_in + k * N + nb.at(-cx27(q), -cy27(q), -cz27(q)));
+            cp_async_elem<real>(stage + (54 + k) * kBlock + tid, src_of(A.f_in, QT, k, q));
         });
     }
     cp_async_commit();
@@ -379,7 +394,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
         if (active) {
 #pragma unroll
-            for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = h[q];
+            for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.h_out, 27, q, q, wl) = h[q]; }
             A.phi_out[cell] = phi_new;
         }
     }
@@ -391,7 +406,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
         if (active) {
 #pragma unroll
-            for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
+            for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.g_out, 27, q, q, wl) = g[q]; }
             A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
         }
     }
@@ -401,7 +416,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         static_for<0, QT>([&](auto K) {
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
             int face = 0;
-            const int ax = nb.crossed(-cx27(q), -cy27(q), -cz27(q), face);
+            const int ax = aa == 1 ? -1 : nb.crossed(-cx27(q), -cy27(q), -cz27(q), face);
             const real v = stage[(54 + k) * kBlock + tid];
             if (WALLS && ax >= 0)   // anti-bounce-back (S9): the staged value is f~_opp of the own cell
                 f[k] = real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, -cx27(q), -cy27(q), -cz27(q)) - v;
@@ -411,7 +426,19 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         const real qT = A.q_src ? A.q_src[cell] : real(0);
         const real Tn = collide_thermal<real, QT, MODE>(A, f, phi_new, u, qT);
         if (active) {
-            static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
+            static_for<0, QT>([&](auto K) {
+                constexpr int k = decltype(K)::value, q = q_of(QT, k);
+                bool wl;
+                real* dst = dst_of(A.f_out, QT, k, q, wl);
+                real v = f[k];
+                if (WALLS && wl) {   // AA odd step, link into a wall: store what the next (even) step must read,
+                                     // i.e. the anti-bounce-back value -f~_q + 2 w T_w (S9)
+                    int face = 0;
+                    const int ax = nb.crossed(cx27(q), cy27(q), cz27(q), face);
+                    v = real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, cx27(q), cy27(q), cz27(q)) - v;
+                }
+                *dst = v;
+            });
             A.T_out[cell] = Tn;
         }
     }
@@ -467,22 +494,69 @@ __global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
     const long long N = A.ncell;
     const real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
     const real uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    // two-grid: population q of the cell goes to plane q at the cell.  AA: the first step is an even one
+    // and reads in place, so the equilibria are stored already streamed ("pushed"): plane q at x + c_q,
+    // or, for a link into a wall, plane opp(q) at x (for f: as its anti-bounce-back value).
+    Nbh<true> nb;
+    if (A.aa) {
+        const int x = cell % A.nx, t = cell / A.nx;
+        nb.init_xyz(A, x, t % A.ny, t / A.ny);
+    }
+    auto dst_of = [&](real* base, int Q, int k, int q27i, bool& wall_link) -> real* {
+        wall_link = false;
+        if (!A.aa) return base + k * N + cell;
+        int face = 0;
+        wall_link = nb.crossed(cx27(q27i), cy27(q27i), cz27(q27i), face) >= 0;
+        return wall_link ? base + (Q - 1 - k) * N + cell : base + k * N + nb.at(cx27(q27i), cy27(q27i), cz27(q27i));
+    };
     real out[27];
     {
         const real s = A.phi_in[cell];
         const real su[3] = {s * u[0], s * u[1], s * u[2]};
         equilibrium_plus_half_force27<real>(s - real(1.5) * s * uu, u, su, su, out);      // eq. 12
 #pragma unroll
-        for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = out[q];
+        for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.h_out, 27, q, q, wl) = out[q]; }
     }
     equilibrium_plus_half_force27<real>(-real(1.5) * uu, u, u, u, out);                   // eq. 18, p* = 0
 #pragma unroll
-    for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = out[q];
+    for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.g_out, 27, q, q, wl) = out[q]; }
     if constexpr (QT > 0) {
         real f[QT];
         thermal_equilibrium<real, QT>(A.T_in[cell], u, f);
-        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
+        static_for<0, QT>([&](auto K) {
+            constexpr int k = decltype(K)::value, q = q_of(QT, k);
+            bool wl;
+            real* dst = dst_of(A.f_out, QT, k, q, wl);
+            real v = f[k];
+            if (wl) {
+                int face = 0;
+                const int ax = nb.crossed(cx27(q), cy27(q), cz27(q), face);
+                v = real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, cx27(q), cy27(q), cz27(q)) - v;
+            }
+            *dst = v;
+        });
     }
+}
+
+// p = c_s^2 rho(phi) sum_q g~_q(x).  pushed = 1: AA layout after init / an odd step, where g~_q(x) sits in
+// plane q at x + c_q (plane opp(q) at x for a link into a wall).
+template <typename real>
+__global__ void __launch_bounds__(kBlock) pressure_pushed_kernel(const StepArgs<real> A, const real* __restrict__ g, const real* __restrict__ phi,
+                                                                real* __restrict__ p) {
+    const int cell = blockIdx.x * kBlock + threadIdx.x;
+    if (cell >= A.ncell) return;
+    const long long N = A.ncell;
+    Nbh<true> nb;
+    const int x = cell % A.nx, t = cell / A.nx;
+    nb.init_xyz(A, x, t % A.ny, t / A.ny);
+    real s = real(0);
+#pragma unroll
+    for (int q = 0; q < 27; ++q) {
+        int face = 0;
+        const bool wl = nb.crossed(cx27(q), cy27(q), cz27(q), face) >= 0;
+        s += wl ? g[(26 - q) * N + cell] : g[q * N + nb.at(cx27(q), cy27(q), cz27(q))];
+    }
+    p[cell] = real(1.0 / 3.0) * (A.rho_L + phi[cell] * A.drho) * s;
 }
 
 template <typename real>

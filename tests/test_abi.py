@@ -44,6 +44,9 @@ def test_workspace_bytes_accounting():
     for thermal, extra in (("lb_d3q7", 14), ("lb_d3q27", 54), ("rk2", 1), ("rk4", 3)):
         for prec, es in (("f64", 8), ("f32", 4)):
             b = tcp.tcp_workspace_bytes(n, n, n, tcp.make_params(dict(thermal=thermal, precision=prec)))
+            aa = tcp.tcp_workspace_bytes(n, n, n, tcp.make_params(dict(thermal=thermal, precision=prec, streaming="aa")))
+            pops = 54 + (extra // 2 if thermal.startswith("lb") else 0)
+            assert abs((b - aa) - pops * N * es) <= 64 * 256      # AA keeps one grid of populations
             fields = 108 + extra + 2 + 2 + 3 + 1            # h, g (x2 grids), thermal, phi x2, T x2, u, q
             planes = 6 * n * n
             assert fields * N * es + planes * es <= b <= fields * N * es + planes * es + 64 * 256
@@ -52,7 +55,6 @@ def test_workspace_bytes_accounting():
 @pytest.mark.parametrize("bad, code", [
     (dict(M=0.0), tcp.TCP_EINVAL), (dict(xi=-1.0), tcp.TCP_EINVAL), (dict(tau_H=-0.5), tcp.TCP_EINVAL),
     (dict(rho_L=0.0), tcp.TCP_EINVAL), (dict(kappa_H=0.0), tcp.TCP_EINVAL),
-    (dict(streaming="aa"), tcp.TCP_EUNSUPPORTED),
 ])
 def test_parameter_validation(bad, code):
     with pytest.raises(tcp.TcpError) as e:

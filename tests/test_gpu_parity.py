@@ -108,6 +108,18 @@ def test_heat_source_and_gravity():
         _check(wl, q=q, extra=dict(gravity=(1e-6, -2e-6, 3e-6), rho_H=4.0))
 
 
+@pytest.mark.parametrize("thermal", ["lb_d3q7", "rk2"])
+def test_laser_heated_droplet_in_channel(thermal):
+    """Droplet-capture ingredients that are in scope: a droplet near a no-slip wall,
+    T = T_ref on both walls, and the laser source q_T of eq. 37 (w_s = 6, d_s = 8 scaled to the box)
+    driving the Marangoni flow; the moving wall and the wetting condition are NEXT-1."""
+    wl = W.thermal_tweezer(nx=36, ny=20, nz=18, thermal=thermal, R=5.0, offset=7.0, A=0.0, s=4.0)
+    q = W.laser_source(36, 20, 18, Q_s=0.02, centre=(14.0, 9.5, 6.0), w_s=4.0, d_s=5.0)
+    assert 0 < int((q > 0).sum()) < q.numel() // 4
+    got, want = _check(wl, q=q.numpy())
+    assert want[3].max() > 0.05                       # the laser did heat the fluid
+
+
 @pytest.mark.parametrize("bc", [("walls", "walls", "periodic"), ("walls", "walls", "walls"), ("walls", "periodic", "periodic")])
 def test_walls_on_several_axes(bc):
     """Corner ghosts / corner links (reading S17) and x-walls."""

@@ -61,6 +61,21 @@ def test_heat_sinusoid_decay_and_advection(thermal, axis):
 
 
 @pytest.mark.parametrize("thermal", THERMALS)
+def test_uniform_heat_source_raises_temperature_linearly(thermal):
+    """q_T of eqs. 4 / 27 on a uniform, quiescent periodic box: dT/dt = q exactly.  RK: T^n = T0 + n q.
+    LB: the + w_i q_T of eq. 27 is added after the collision, so it shows in T = sum f one step later:
+    T^n = T0 + (n - 1) q."""
+    n, q, T0, steps = 6, 2.5e-3, 0.7, 40
+    o = tcpo.Oracle(n, n, n, dict(thermal=thermal, xi=1e30))
+    o.set_heat_source(np.full((n, n, n), q))
+    o.init_fields(np.zeros((n, n, n)), T=np.full((n, n, n), T0))
+    o.step(steps)
+    T = o.read_fields()[3]
+    expect = T0 + (steps - 1 if thermal.startswith("lb") else steps) * q
+    assert np.abs(T - expect).max() < 1e-12
+
+
+@pytest.mark.parametrize("thermal", THERMALS)
 def test_two_wall_conduction_is_linear_through_wall_values(thermal):
     """S9: Dirichlet walls half a cell outside the end cells; steady profile linear and equal to
     T_w at y = -1/2 and y = ny - 1/2, also across a conductivity jump-free slab."""

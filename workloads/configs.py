@@ -221,3 +221,21 @@ def perf_box(n, thermal="lb_d3q7", seed=None, device="cpu", nz=None, ny=None, vo
     wl = Workload(f"perf_box_{nx}x{ny}x{nz}", nx, ny, nz, params, phi, T=T, steps=100)
     wl.notes = f"{len(radii)} droplets, seed {seed}"
     return wl
+
+
+# --------------------------------------------------------------------------------------------
+# laser heat source of the droplet-capture set-ups (eq. 37)
+
+def laser_source(nx, ny, nz, Q_s=0.2, centre=None, w_s=6.0, d_s=8.0):
+    """q_T = Q_s exp(-2 r^2 / w_s^2) where r^2 <= d_s^2, 0 elsewhere (eq. 37 in reading G9: the printed
+    ">= d_s^2" would switch the source on everywhere EXCEPT around the laser).  `centre` = (x_s, y_s, z_s) in
+    cell coordinates; for nz = 1 the z component is ignored as in the paper's 2-D cases."""
+    if centre is None:
+        centre = ((nx - 1) / 2.0, (ny - 1) / 2.0, (nz - 1) / 2.0)
+    x, y, z = _grid(nx, ny, nz)
+    r2 = (x - centre[0]) ** 2 + (y - centre[1]) ** 2
+    if nz > 1:
+        r2 = r2 + (z - centre[2]) ** 2
+    r2 = r2.expand(nz, ny, nx)
+    q = Q_s * torch.exp(-2.0 * r2 / (w_s * w_s))
+    return torch.where(r2 <= d_s * d_s, q, torch.zeros_like(q)).contiguous()

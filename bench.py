@@ -203,6 +203,11 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     ms_max = max_over_ranks(ms, dist)
     value = aggregate_mlups(N, args.steps, world, ms_max)
+    # roofline calibration: the same access pattern and staging with stencils and collisions removed
+    pattern_ms = None
+    if rank == 0 and args.streaming == "two_grid":
+        sim.pattern_copy_ms(3)
+        pattern_ms = sim.pattern_copy_ms(max(5, min(args.steps, 20)))
     phi_chk = sim.read_fields_device()[0]
     finite = bool(torch.isfinite(phi_chk).all().item())
     sum_drift = abs(float(phi_chk.double().sum().item()) - float(phi_d.double().sum().item())) / float(phi_d.double().sum().item())
@@ -248,7 +253,10 @@ def run_ours(args):
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": recorded_traffic(f"{thermal}_{prec}_{n}"), "kernel": kname, "peak_source": peak_src,
                 "algorithmic_bytes_per_cell": (fused_bytes if QT[thermal] else step_bytes) / N,
-                "kernel_ms": k_ms}
+                "kernel_ms": k_ms,
+                # what a no-arithmetic kernel with the fused kernel's pulls, staging and stores reaches on this GPU
+                "pattern_copy": None if pattern_ms is None else {"ms": pattern_ms, "gbs": fused_bytes / (pattern_ms * 1e-3) / 1e9,
+                                                                  "frac_of_peak": fused_bytes / (pattern_ms * 1e-3) / 1e9 / peak}}
     cpu = None
     if not args.no_cpu:
         v, _, cores, sample = oracle_throughput(thermal)

@@ -107,6 +107,13 @@ long long tcp_launch_count(const tcp_sim *s);
  * Errors: TCP_ESTATE if tcp_step has not been called. */
 int tcp_last_step_ms(tcp_sim *s, float *ms);
 
+/* Roofline calibration, not part of the method: launch `nlaunches` times a kernel with exactly the memory
+ * access pattern and staging of the fused step (same pulls, same stores) but no stencils and no collision,
+ * and return its mean duration.  It reads the current state and overwrites only the spare grid and the
+ * spare phi / T buffers, so the simulation is unchanged -- except u, which is rewritten with itself.
+ * Errors: TCP_ESTATE, TCP_EINVAL, TCP_EUNSUPPORTED (walls or AA streaming). */
+int tcp_pattern_copy_ms(tcp_sim *s, int nlaunches, float *ms);
+
 int tcp_destroy(tcp_sim *s);
 
 const char *tcp_last_error(void);

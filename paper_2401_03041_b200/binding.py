@@ -74,7 +74,7 @@ def make_params(d: dict) -> tcp_params:
 
 EXPORTS = ["tcp_workspace_bytes", "tcp_create", "tcp_create_in", "tcp_init_fields", "tcp_set_wall_temperature",
            "tcp_set_heat_source", "tcp_step", "tcp_read_fields", "tcp_synchronize", "tcp_launch_count",
-           "tcp_last_step_ms", "tcp_destroy", "tcp_last_error"]
+           "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_destroy", "tcp_last_error"]
 
 _lib = None
 
@@ -102,6 +102,7 @@ def lib():
         L.tcp_launch_count.argtypes = [vp]
         L.tcp_launch_count.restype = C.c_longlong
         L.tcp_last_step_ms.argtypes = [vp, C.POINTER(C.c_float)]
+        L.tcp_pattern_copy_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
         L.tcp_destroy.argtypes = [vp]
         L.tcp_last_error.restype = C.c_char_p
         _lib = L
@@ -186,6 +187,12 @@ def tcp_last_step_ms(sim) -> float:
     return float(ms.value)
 
 
+def tcp_pattern_copy_ms(sim, nlaunches=10) -> float:
+    ms = C.c_float()
+    _check(lib().tcp_pattern_copy_ms(sim, int(nlaunches), C.byref(ms)))
+    return float(ms.value)
+
+
 def tcp_destroy(sim):
     _check(lib().tcp_destroy(sim))
 
@@ -256,6 +263,9 @@ class Simulation:
 
     def last_step_ms(self):
         return tcp_last_step_ms(self._h)
+
+    def pattern_copy_ms(self, nlaunches=10):
+        return tcp_pattern_copy_ms(self._h, nlaunches)
 
     def close(self):
         if getattr(self, "_h", None):

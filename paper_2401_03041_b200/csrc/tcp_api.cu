@@ -476,6 +476,28 @@ int tcp_synchronize(tcp_sim* s) {
 
 long long tcp_launch_count(const tcp_sim* s) { return s ? s->launches : 0; }
 
+int tcp_pattern_copy_ms(tcp_sim* s, int nlaunches, float* ms) {
+    if (!s || !ms) return fail(TCP_EINVAL, "NULL argument");
+    if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
+    if (nlaunches < 1) return fail(TCP_EINVAL, "nlaunches must be >= 1");
+    if (s->walls || s->P.streaming != TCP_STREAM_TWO_GRID) return fail(TCP_EUNSUPPORTED, "pattern copy: periodic two-grid simulations only");
+    tcp::FusedCfg c;
+    c.qt = thermal_q(s->P.thermal); c.walls = false; c.mode = 3; c.aa = 0; c.staged = true; c.grid = grid_for(s->N);
+    CK(cudaEventRecord(s->ev0, s->stream));
+    for (int i = 0; i < nlaunches; ++i) {
+        // in -> out only: the simulation's current state (grid `cur`) is read, the spare grid is overwritten
+        if (s->P.precision == TCP_F64) CK(tcp::launch_fused_periodic(c, make_args<double>(s), s->stream));
+        else CK(tcp::launch_fused_periodic(c, make_args<float>(s), s->stream));
+        s->launches++;
+    }
+    CK(cudaEventRecord(s->ev1, s->stream));
+    CK(cudaEventSynchronize(s->ev1));
+    float total = 0.f;
+    CK(cudaEventElapsedTime(&total, s->ev0, s->ev1));
+    *ms = total / nlaunches;
+    return TCP_OK;
+}
+
 int tcp_last_step_ms(tcp_sim* s, float* ms) {
     if (!s || !ms) return fail(TCP_EINVAL, "NULL argument");
     if (!s->stepped) return fail(TCP_ESTATE, "tcp_step has not been called");

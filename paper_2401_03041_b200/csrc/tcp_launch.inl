@@ -21,6 +21,10 @@ cudaError_t dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t st
         fused_step_kernel<real, QT, WALLS, 0><<<c.grid, kBlock, 0, stream>>>(A);
         return cudaGetLastError();
     }
+    if (c.mode == 3) {   // roofline calibration kernel (tcp_pattern_copy_ms): two-grid, periodic only
+        if constexpr (!WALLS) return launch_staged<real, QT, false, 3, 0>(c, A, stream);
+        else return cudaErrorNotSupported;
+    }
     switch (3 * c.aa + c.mode) {   // c.aa: 0 two-grid, 1 AA even step, 2 AA odd step
     case 0: return launch_staged<real, QT, WALLS, 0, 0>(c, A, stream);
     case 1: return launch_staged<real, QT, WALLS, 1, 0>(c, A, stream);

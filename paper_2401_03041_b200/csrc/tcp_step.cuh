@@ -383,9 +383,16 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
     }
     cp_async_commit();
 
+    // MODE 3 is a roofline calibration, not a step of the method: same pulls, staging and stores, but the
+    // stencils and collisions are left out (h, g, f are streamed unchanged; phi, T, u copied through).
     real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
-    stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
-    stencil27<real, WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
+    if constexpr (MODE == 3) {
+        phi_c = A.phi_in[cell]; T_c = A.T_in[cell];
+        G[0] = G[1] = G[2] = Th[0] = Th[1] = Th[2] = lapPhi = lapT = real(0);
+    } else {
+        stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
+        stencil27<real, WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
+    }
     real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
 
     real phi_new;
@@ -394,7 +401,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         real h[27];
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = stage[q * kBlock + tid];
-        phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
+        if constexpr (MODE == 3) phi_new = phi_c; else phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
         if (active) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.h_out, 27, q, q, wl) = h[q]; }
@@ -406,7 +413,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         real g[27];
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = stage[(27 + q) * kBlock + tid];
-        collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+        if constexpr (MODE != 3) collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
         if (active) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.g_out, 27, q, q, wl) = g[q]; }
@@ -427,7 +434,8 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
                 f[k] = v;
         });
         const real qT = A.q_src ? A.q_src[cell] : real(0);
-        const real Tn = collide_thermal<real, QT, MODE>(A, f, phi_new, u, qT);
+        real Tn;
+        if constexpr (MODE == 3) Tn = T_c + qT; else Tn = collide_thermal<real, QT, MODE>(A, f, phi_new, u, qT);
         if (active) {
             static_for<0, QT>([&](auto K) {
                 constexpr int k = decltype(K)::value, q = q_of(QT, k);

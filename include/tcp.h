@@ -58,6 +58,8 @@ typedef struct tcp_params {
                                           full central-moment transform (about 25 % more instructions) */
     int high_rate_equals_shear;        /* 1: every rate = the physical one = plain BGK + Guo */
     double eps_normal;                 /* n = grad phi / sqrt(|grad phi|^2 + eps); default 1e-32 */
+    double wall_u[3][2][3];            /* velocity of each wall [axis][face][component] (moving wall):
+                                          enters the bounce-back of g only; default 0 */
 } tcp_params;
 
 /* Bytes of device memory one simulation needs (populations, fields, wall planes).

@@ -56,6 +56,7 @@ typedef struct tcpo_params {
     double s_bulk, s_high;             /* reading S2 */
     int high_rate_equals_shear;        /* 1 => every rate = the physical one => BGK */
     double eps_normal;                 /* reading S8 */
+    double wall_u[3][2][3];            /* wall velocity per axis / face (moving wall; reading S18) */
 } tcpo_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -480,6 +481,19 @@ static double pull_bb(const tcpo_sim *s, const lattice *L, const double *a, int 
     return a[(size_t)i * s->N + r.idx];
 }
 
+/* hydrodynamic pull: halfway bounce-back from a wall moving with U_w (reading S18):
+ *   g_i(x) = g~_ibar(x) + 2 w_i (c_i . U_w) / c_s^2   (velocity-based model: no density factor);
+ * h and f keep the plain (anti-)bounce-back of S9 */
+static double pull_bb_moving(const tcpo_sim *s, const lattice *L, const double *a, int i, int x, int y, int z, size_t k) {
+    nbr r = neighbour(s, x, y, z, -L->c[i][0], -L->c[i][1], -L->c[i][2]);
+    if (r.axis >= 0) {
+        const double *U = s->P.wall_u[r.axis][r.face];
+        double cu = L->c[i][0] * U[0] + L->c[i][1] * U[1] + L->c[i][2] * U[2];
+        return a[(size_t)L->opp[i] * s->N + k] + 2.0 * L->w[i] * cu / CS2;
+    }
+    return a[(size_t)i * s->N + r.idx];
+}
+
 /* thermal pull: Dirichlet wall by anti-bounce-back  -f~_ibar(x) + 2 w_i T_w */
 static double pull_abb(const tcpo_sim *s, const lattice *L, const double *a, int i, int x, int y, int z, size_t k) {
     nbr r = neighbour(s, x, y, z, -L->c[i][0], -L->c[i][1], -L->c[i][2]);
@@ -547,7 +561,7 @@ static int update_g(tcpo_sim *s) {
                 double gp[QMAX], geq[QMAX], gout[QMAX];
                 double pstar = 0.0, j[3] = {0, 0, 0};
                 for (int i = 0; i < 27; i++) { /* O4, eq. 17 */
-                    gp[i] = pull_bb(s, L, s->g, i, x, y, z, k);
+                    gp[i] = pull_bb_moving(s, L, s->g, i, x, y, z, k);
                     pstar += gp[i];
                     for (int al = 0; al < 3; al++) j[al] += L->c[i][al] * gp[i];
                 }
@@ -690,6 +704,20 @@ int tcpo_step(tcpo_sim *s, int nsteps) {
         { double *t = s->phi; s->phi = s->phi2; s->phi2 = t; } /* phi^{n+1} becomes current (S16) */
         if ((rc = s->thermal_is_lb ? update_f(s) : update_T_rk(s))) return rc;
         s->steps_done++;
+    }
+    return TCPO_OK;
+}
+
+/* Temperature pre-initialisation ("the temperature field is often times initialised by
+ * executing the thermal solver until a certain error is reached"): the temperature update alone, with
+ * phi, u, h~, g~ frozen. */
+int tcpo_relax_temperature(tcpo_sim *s, int nsteps) {
+    if (!s) return fail(TCPO_EINVAL, "null sim");
+    if (!s->initialised) return fail(TCPO_ESTATE, "tcpo_init_fields not called");
+    if (nsteps < 0) return fail(TCPO_EINVAL, "nsteps < 0");
+    for (int n = 0; n < nsteps; n++) {
+        int rc = s->thermal_is_lb ? update_f(s) : update_T_rk(s);
+        if (rc) return rc;
     }
     return TCPO_OK;
 }

@@ -30,6 +30,7 @@ class Params(C.Structure):
         ("s_bulk", C.c_double), ("s_high", C.c_double),
         ("high_rate_equals_shear", C.c_int),
         ("eps_normal", C.c_double),
+        ("wall_u", ((C.c_double * 3) * 2) * 3),
     ]
 
 
@@ -40,6 +41,7 @@ DEFAULTS = dict(
     kappa_H=0.2, kappa_L=0.2, cp_H=1.0, cp_L=1.0,
     gravity=(0.0, 0.0, 0.0), wall_T=((0.0, 0.0), (0.0, 0.0), (0.0, 0.0)),
     s_bulk=1.0, s_high=1.0, high_rate_equals_shear=0, eps_normal=1e-32,
+    wall_u=(((0.0,) * 3,) * 2,) * 3,
 )
 
 
@@ -65,6 +67,10 @@ def make_params(d: dict) -> Params:
               "kappa_H", "kappa_L", "cp_H", "cp_L", "s_bulk", "s_high", "eps_normal"):
         setattr(p, k, float(v[k]))
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
+    for a in range(3):
+        for f in range(2):
+            for c in range(3):
+                p.wall_u[a][f][c] = float(v["wall_u"][a][f][c])
     return p
 
 
@@ -84,6 +90,7 @@ def lib():
         L.tcpo_set_wall_temperature.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
         L.tcpo_set_heat_source.argtypes = [C.c_void_p, dp]
         L.tcpo_step.argtypes = [C.c_void_p, C.c_int]
+        L.tcpo_relax_temperature.argtypes = [C.c_void_p, C.c_int]
         L.tcpo_read_fields.argtypes = [C.c_void_p, dp, dp, dp, dp]
         L.tcpo_read_populations.argtypes = [C.c_void_p, C.c_int, dp]
         L.tcpo_lattice.argtypes = [C.c_int, ip, dp, ip, ip]
@@ -156,6 +163,9 @@ class Oracle:
 
     def step(self, n=1):
         _check(lib().tcpo_step(self._h, int(n)))
+
+    def relax_temperature(self, n=1):
+        _check(lib().tcpo_relax_temperature(self._h, int(n)))
 
     def read_fields(self):
         nz, ny, nx = self.shape

@@ -35,6 +35,7 @@ class tcp_params(C.Structure):
         ("s_bulk", C.c_double), ("s_high", C.c_double),
         ("high_rate_equals_shear", C.c_int),
         ("eps_normal", C.c_double),
+        ("wall_u", ((C.c_double * 3) * 2) * 3),
     ]
 
 
@@ -45,6 +46,7 @@ PARAM_DEFAULTS = dict(
     kappa_H=0.2, kappa_L=0.2, cp_H=1.0, cp_L=1.0,
     gravity=(0.0, 0.0, 0.0), wall_T=((0.0, 0.0), (0.0, 0.0), (0.0, 0.0)),
     s_bulk=1.0, s_high=1.0, high_rate_equals_shear=0, eps_normal=1e-32,
+    wall_u=(((0.0,) * 3,) * 2,) * 3,
 )
 
 
@@ -69,6 +71,10 @@ def make_params(d: dict) -> tcp_params:
               "kappa_H", "kappa_L", "cp_H", "cp_L", "s_bulk", "s_high", "eps_normal"):
         setattr(p, k, float(v[k]))
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
+    for a in range(3):
+        for f in range(2):
+            for c in range(3):
+                p.wall_u[a][f][c] = float(v["wall_u"][a][f][c])
     return p
 
 

@@ -280,3 +280,66 @@ def test_droplet_migrates_toward_hot_wall():
         assert abs(phi.sum() - float(wl.phi.sum())) / float(wl.phi.sum()) < 1e-12
     assert zc["lb_d3q19"] - 17.0 > 0.02
     assert zc["lb_d3q19"] == pytest.approx(zc["rk4"], abs=1e-3)
+
+
+# ---- NEXT-1 ingredients: moving wall and temperature pre-initialisation ----
+
+def _wall_u(axis, face, vec):
+    w = [[[0.0] * 3 for _ in range(2)] for _ in range(3)]
+    w[axis][face] = list(vec)
+    return w
+
+
+def test_couette_flow_from_a_moving_wall():
+    """Top wall moving with U_w, bottom wall at rest (reading S18: velocity bounce-back on g):
+    steady u(y) = U_w (y + 1/2) / H, walls half a cell outside the end cells."""
+    ny, U, nu = 16, 0.01, 0.2
+    o = tcpo.Oracle(3, ny, 2, dict(bc=("periodic", "walls", "periodic"), tau_H=3 * nu, tau_L=3 * nu, xi=1e30,
+                                   wall_u=_wall_u(1, 1, (U, 0.0, 0.0))))
+    o.init_fields(np.zeros((2, ny, 3)))
+    o.step(7000)
+    u = o.read_fields()[1]
+    exact = U * (np.arange(ny) + 0.5) / ny
+    assert np.abs(u[0, 0, :, 0] - exact).max() < 1e-8
+    assert np.abs(u[1:]).max() < 1e-15
+
+
+def test_two_layer_couette_with_viscosity_contrast():
+    """Two layers with nu_H / nu_L = 4 (tau interpolated by phi, eq. 22) sheared by a moving top wall:
+    the stress mu du/dy is uniform, so the sharp-interface profile is piecewise linear with slopes in the
+    ratio nu_L / nu_H."""
+    ny, U = 32, 0.01
+    wl = W.layered_channel(nx=1, ny=ny, nz=1)
+    wl.params.update(sigma_T=0.0, sigma_ref=0.0, tau_H=1.2, tau_L=0.3, wall_u=_wall_u(1, 1, (U, 0.0, 0.0)))
+    o = tcpo.Oracle(1, ny, 1, wl.params)
+    o.init_fields(wl.phi.numpy(), T=np.full((1, ny, 1), 10.0))
+    o.step(15000)
+    u = o.read_fields()[1][0].ravel()
+    h = ny / 2.0
+    nuL, nuH = 0.3 / 3, 1.2 / 3                       # lower layer = L, upper = H
+    sL = U / (h + h * nuL / nuH)                      # slope in the lower layer; upper slope = sL nuL / nuH
+    yy = np.arange(ny) + 0.5
+    exact = np.where(yy < h, sL * yy, sL * h + sL * nuL / nuH * (yy - h))
+    assert np.abs(u - exact).max() / U < 0.04          # diffuse interface (xi = 4) rounds the kink
+    slope_lo = (u[8] - u[2]) / 6.0
+    slope_up = (u[29] - u[23]) / 6.0
+    assert slope_lo / slope_up == pytest.approx(nuH / nuL, rel=0.03)     # uniform shear stress
+
+
+@pytest.mark.parametrize("thermal", ["lb_d3q7", "lb_d3q19", "rk2", "rk4"])
+def test_temperature_preinitialisation_reaches_steady_conduction(thermal):
+    """tcpo_relax_temperature: the thermal solver alone, phi / u / h / g frozen, relaxes a uniform initial
+    temperature to the steady conduction field of the heated channel, App. A (k* = 1: harmonic T)."""
+    nx, ny = 32, 16
+    wl = W.layered_channel(nx, ny, 1, thermal=thermal)
+    o = tcpo.Oracle(nx, ny, 1, wl.params)
+    for (ax, fc), v in wl.wall_T.items():
+        o.set_wall_temperature(ax, fc, v.numpy())
+    o.init_fields(wl.phi.numpy(), T=np.full((1, ny, nx), 15.0))
+    h0, g0 = o.read_populations(0), o.read_populations(1)
+    o.relax_temperature(2500)
+    phi, u, p, T = o.read_fields()
+    Ta = wl.T.numpy()
+    assert np.sqrt(((T - Ta) ** 2).sum() / (Ta ** 2).sum()) < 1e-3
+    assert np.array_equal(h0, o.read_populations(0)) and np.array_equal(g0, o.read_populations(1))
+    assert np.array_equal(phi, wl.phi.numpy()) and np.abs(u).max() == 0.0

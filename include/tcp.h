@@ -94,6 +94,12 @@ int tcp_set_heat_source(tcp_sim *s, const void *q);
  * Errors: TCP_ESTATE (fields not initialised), TCP_EINVAL (nsteps < 0), TCP_ECUDA. */
 int tcp_step(tcp_sim *s, int nsteps);
 
+/* Temperature pre-initialisation (the temperature field is often initialised by running the
+ * thermal solver to convergence): nsteps temperature updates alone (thermal LB, or the RK stages), with phi,
+ * u and the phase-field / hydrodynamic populations frozen.  With TCP_STREAM_AA and a thermal LB nsteps must
+ * be even.  Errors: TCP_ESTATE, TCP_EINVAL, TCP_ECUDA. */
+int tcp_relax_temperature(tcp_sim *s, int nsteps);
+
 /* Copy out phi, u, p = c_s^2 rho(phi) sum_i g~_i, T; any pointer may be NULL.
  * Synchronises the stream. */
 int tcp_read_fields(tcp_sim *s, void *phi, void *u, void *p, void *T);

@@ -79,7 +79,7 @@ def make_params(d: dict) -> tcp_params:
 
 
 EXPORTS = ["tcp_workspace_bytes", "tcp_create", "tcp_create_in", "tcp_init_fields", "tcp_set_wall_temperature",
-           "tcp_set_heat_source", "tcp_step", "tcp_read_fields", "tcp_synchronize", "tcp_launch_count",
+           "tcp_set_heat_source", "tcp_step", "tcp_relax_temperature", "tcp_read_fields", "tcp_synchronize", "tcp_launch_count",
            "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_destroy", "tcp_last_error"]
 
 _lib = None
@@ -103,6 +103,7 @@ def lib():
         L.tcp_set_wall_temperature.argtypes = [vp, C.c_int, C.c_int, vp]
         L.tcp_set_heat_source.argtypes = [vp, vp]
         L.tcp_step.argtypes = [vp, C.c_int]
+        L.tcp_relax_temperature.argtypes = [vp, C.c_int]
         L.tcp_read_fields.argtypes = [vp, vp, vp, vp, vp]
         L.tcp_synchronize.argtypes = [vp]
         L.tcp_launch_count.argtypes = [vp]
@@ -175,6 +176,10 @@ def tcp_step(sim, nsteps=1):
     _check(lib().tcp_step(sim, int(nsteps)))
 
 
+def tcp_relax_temperature(sim, nsteps=1):
+    _check(lib().tcp_relax_temperature(sim, int(nsteps)))
+
+
 def tcp_read_fields(sim, phi=None, u=None, p=None, T=None):
     _check(lib().tcp_read_fields(sim, _ptr(phi), _ptr(u), _ptr(p), _ptr(T)))
 
@@ -244,6 +249,9 @@ class Simulation:
 
     def step(self, n=1):
         tcp_step(self._h, n)
+
+    def relax_temperature(self, n=1):
+        tcp_relax_temperature(self._h, n)
 
     def read_fields(self):
         """-> phi, u, p, T as host numpy arrays in the simulation's precision."""

@@ -109,7 +109,8 @@ struct tcp_sim {
     char* base;
     bool owns_memory, owns_stream;
     cudaStream_t stream;
-    int cur;                 // index of the buffers holding time level n
+    int cur;                 // index of the h, g, phi buffers holding time level n
+    int curT;                // same for f and T (they advance alone in tcp_relax_temperature)
     bool initialised, has_q, walls, stepped;
     long long launches;
     cudaEvent_t ev0, ev1;
@@ -130,16 +131,16 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     tcp::StepArgs<real> A;
     std::memset(&A, 0, sizeof A);
     const tcp_params& P = s->P;
-    const int c = s->cur, o = 1 - s->cur;
+    const int c = s->cur, o = 1 - s->cur, cT = s->curT, oT = 1 - s->curT;
     A.nx = s->nx; A.ny = s->ny; A.nz = s->nz; A.ncell = (int)s->N;
     A.bz = s->bz;
     A.aa = s->aa_next;
     for (int a = 0; a < 3; ++a) A.wall[a] = P.bc[a] == TCP_BC_WALLS;
     A.h_in = ptr<real>(s, s->L.h[c]); A.h_out = ptr<real>(s, s->L.h[o]);
     A.g_in = ptr<real>(s, s->L.g[c]); A.g_out = ptr<real>(s, s->L.g[o]);
-    A.f_in = ptr<real>(s, s->L.f[c]); A.f_out = ptr<real>(s, s->L.f[o]);
+    A.f_in = ptr<real>(s, s->L.f[cT]); A.f_out = ptr<real>(s, s->L.f[oT]);
     A.phi_in = ptr<real>(s, s->L.phi[c]); A.phi_out = ptr<real>(s, s->L.phi[o]);
-    A.T_in = ptr<real>(s, s->L.T[c]); A.T_out = ptr<real>(s, s->L.T[o]);
+    A.T_in = ptr<real>(s, s->L.T[cT]); A.T_out = ptr<real>(s, s->L.T[oT]);
     A.u = ptr<real>(s, s->L.u);
     A.q_src = s->has_q ? ptr<real>(s, s->L.q) : nullptr;
     for (int a = 0; a < 3; ++a)
@@ -153,6 +154,13 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     for (int a = 0; a < 3; ++a) A.grav[a] = (real)P.gravity[a];
     A.s_bulk = (real)P.s_bulk;
     A.s_high = (real)P.s_high;
+    A.moving = 0;
+    for (int a = 0; a < 3; ++a)
+        for (int fc = 0; fc < 2; ++fc)
+            for (int k = 0; k < 3; ++k) {
+                A.wall_u[a][fc][k] = (real)P.wall_u[a][fc][k];
+                if (P.wall_u[a][fc][k] != 0.0) A.moving = 1;
+            }
     // S8: eps keeps n = grad phi / |grad phi| finite where grad phi vanishes.  In fp32 a gradient
     // below ~1e-6 is round-off of phi ~ 1, and a round-off-directed sharpening flux makes phi = 0 / 1
     // unstable to noise (measured: 1e-4 error after 100 steps next to a wall), so eps is floored there.
@@ -200,35 +208,17 @@ int launch_rows(const tcp_sim* s, const tcp::StepArgs<real>& A) {
 
 #endif
 
-// one time step: Algorithm 1 (thermal LB, one fused kernel) or Algorithm 2 (fused phase+hydro
-// kernel, then the Runge-Kutta stages), PAPER.md:361-390
+// Runge-Kutta update of T (eqs. 25-26) from T[curT] into T[1 - curT]; phi = the phi to differentiate
 template <typename real>
-int step_once(tcp_sim* s) {
-    tcp::StepArgs<real> A = make_args<real>(s);
-    // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
-    const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
-    {
-        tcp::FusedCfg c;
-        c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
-        c.staged = s->use_async || mode != 0 || c.aa != 0;
-        c.grid = grid_for(s->N);
-#ifdef TCP_EXPERIMENTAL_ROWS
-        if (!c.staged && s->use_rows) {
-            int rc = s->walls ? launch_rows<real, true>(s, A) : launch_rows<real, false>(s, A);
-            if (rc) return rc;
-        } else
-#endif
-        CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
-    }
-    s->launches++;
+void rk_update(tcp_sim* s, const tcp::StepArgs<real>& A, const real* phi) {
     const int th = s->P.thermal;
     if (th == TCP_THERMAL_RK2 || th == TCP_THERMAL_RK4) {
         tcp::RkArgs<real> R;
         std::memset(&R, 0, sizeof R);
         R.S = A;
-        R.S.phi_in = A.phi_out;              // phi^{n+1}; u already holds u^{n+1}
-        real* Tn = ptr<real>(s, s->L.T[s->cur]);
-        real* Tnew = ptr<real>(s, s->L.T[1 - s->cur]);
+        R.S.phi_in = phi;
+        real* Tn = ptr<real>(s, s->L.T[s->curT]);
+        real* Tnew = ptr<real>(s, s->L.T[1 - s->curT]);
         real* Ya = ptr<real>(s, s->L.rk[0]);
         R.Tn = Tn;
         if (th == TCP_THERMAL_RK2) {         // eq. 26 (G6)
@@ -252,7 +242,54 @@ int step_once(tcp_sim* s) {
             s->launches += 4;
         }
     }
+}
+
+// temperature update alone, phi / u / h~ / g~ frozen
+template <typename real>
+int relax_t(tcp_sim* s, int nsteps) {
+    const int qt = thermal_q(s->P.thermal);
+    int aa = s->aa_next;                       // parity of the thermal populations during the relaxation
+    for (int n = 0; n < nsteps; ++n) {
+        tcp::StepArgs<real> A = make_args<real>(s);
+        if (qt) {
+            tcp::FusedCfg c;
+            c.qt = qt; c.walls = s->walls; c.mode = s->P.high_rate_equals_shear ? 1 : 0; c.aa = aa; c.staged = true; c.grid = grid_for(s->N);
+            CK(s->walls ? tcp::launch_thermal_walls(c, A, s->stream) : tcp::launch_thermal_periodic(c, A, s->stream));
+            s->launches++;
+            if (aa) aa = 3 - aa;
+        } else {
+            rk_update<real>(s, A, A.phi_in);
+        }
+        s->curT = 1 - s->curT;
+    }
+    CK(cudaGetLastError());
+    return TCP_OK;
+}
+
+// one time step: Algorithm 1 (thermal LB, one fused kernel) or Algorithm 2 (fused phase+hydro
+// kernel, then the Runge-Kutta stages), PAPER.md:361-390
+template <typename real>
+int step_once(tcp_sim* s) {
+    tcp::StepArgs<real> A = make_args<real>(s);
+    // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
+    const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
+    {
+        tcp::FusedCfg c;
+        c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
+        c.staged = s->use_async || mode != 0 || c.aa != 0;
+        c.grid = grid_for(s->N);
+#ifdef TCP_EXPERIMENTAL_ROWS
+        if (!c.staged && s->use_rows) {
+            int rc = s->walls ? launch_rows<real, true>(s, A) : launch_rows<real, false>(s, A);
+            if (rc) return rc;
+        } else
+#endif
+        CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+    }
+    s->launches++;
+    rk_update<real>(s, A, A.phi_out);        // phi^{n+1}; u already holds u^{n+1}
     s->cur = 1 - s->cur;
+    s->curT = 1 - s->curT;
     if (s->aa_next) s->aa_next = 3 - s->aa_next;
     return TCP_OK;
 }
@@ -261,6 +298,7 @@ template <typename real>
 int init_fields_t(tcp_sim* s, const void* phi, const void* u, const void* T) {
     const size_t N = s->N, es = sizeof(real);
     s->cur = 0;
+    s->curT = 0;
     CK(cudaMemcpyAsync(ptr<real>(s, s->L.phi[0]), phi, N * es, cudaMemcpyDefault, s->stream));
     if (u) CK(cudaMemcpyAsync(ptr<real>(s, s->L.u), u, 3 * N * es, cudaMemcpyDefault, s->stream));
     else CK(cudaMemsetAsync(ptr<real>(s, s->L.u), 0, 3 * N * es, s->stream));
@@ -307,7 +345,7 @@ int read_fields_t(tcp_sim* s, void* phi, void* u, void* p, void* T) {
     const size_t N = s->N, es = sizeof(real);
     if (phi) CK(cudaMemcpyAsync(phi, ptr<real>(s, s->L.phi[s->cur]), N * es, cudaMemcpyDefault, s->stream));
     if (u) CK(cudaMemcpyAsync(u, ptr<real>(s, s->L.u), 3 * N * es, cudaMemcpyDefault, s->stream));
-    if (T) CK(cudaMemcpyAsync(T, ptr<real>(s, s->L.T[s->cur]), N * es, cudaMemcpyDefault, s->stream));
+    if (T) CK(cudaMemcpyAsync(T, ptr<real>(s, s->L.T[s->curT]), N * es, cudaMemcpyDefault, s->stream));
     if (p) {
         real* scratch = ptr<real>(s, s->L.phi[1 - s->cur]);   // free between steps
         if (s->aa_next == 1)   // AA, populations in the pushed layout (after init or an odd step)
@@ -459,6 +497,16 @@ int tcp_step(tcp_sim* s, int nsteps) {
     CK(cudaGetLastError());
     s->stepped = true;
     return TCP_OK;
+}
+
+int tcp_relax_temperature(tcp_sim* s, int nsteps) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
+    if (nsteps < 0) return fail(TCP_EINVAL, "nsteps must be >= 0");
+    const bool lb = thermal_q(s->P.thermal) != 0;
+    if (lb && s->P.streaming == TCP_STREAM_AA && (nsteps & 1))
+        return fail(TCP_EINVAL, "AA streaming: the thermal populations must keep the parity of h and g, so nsteps must be even");
+    return s->P.precision == TCP_F64 ? relax_t<double>(s, nsteps) : relax_t<float>(s, nsteps);
 }
 
 int tcp_read_fields(tcp_sim* s, void* phi, void* u, void* p, void* T) {

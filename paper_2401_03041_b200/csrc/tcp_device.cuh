@@ -30,6 +30,8 @@ struct StepArgs {
     real kappa_L, dkappa, cp_L, dcp; // eqs. 23-24 (reading G5)
     real grav[3];                    // eq. 7
     real s_bulk, s_high, eps;
+    int moving;                      // any wall velocity non-zero
+    real wall_u[3][2][3];            // wall velocity [axis][face][component] (moving wall, reading S18)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -106,6 +108,20 @@ template <typename real, bool WALLS>
 __device__ __forceinline__ real wall_temperature(const StepArgs<real>& A, const Nbh<WALLS>& nb, int axis, int face,
                                                  int ox, int oy, int oz) {
     return A.wallT[axis][face][nb.tangential(axis, ox, oy, oz)];
+}
+
+// moving wall (reading S18): a population of direction (cx,cy,cz) that arrives at the cell
+// from a wall moving with U_w is the bounced one plus 2 w (c . U_w) / c_s^2 (hydrodynamic lattice only;
+// velocity-based model, no density factor).  (ox,oy,oz) = direction in which the wall lies (= -c).
+template <typename real, bool WALLS>
+__device__ __forceinline__ real wall_velocity_term(const StepArgs<real>& A, const Nbh<WALLS>& nb, int q27i) {
+    if (!WALLS || !A.moving) return real(0);
+    const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
+    int face = 0;
+    const int ax = nb.crossed(-cx, -cy, -cz, face);
+    if (ax < 0) return real(0);
+    const real* U = A.wall_u[ax][face];
+    return real(6.0 * weight(27, cls27(q27i))) * (real(cx) * U[0] + real(cy) * U[1] + real(cz) * U[2]);
 }
 
 // ---------------------------------------------------------------------------------------------

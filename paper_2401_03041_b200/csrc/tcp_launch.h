@@ -21,4 +21,10 @@ cudaError_t launch_fused_periodic(const FusedCfg& c, const StepArgs<float>& A, c
 cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
 cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
 
+// thermal LB update alone (tcp_relax_temperature); c.mode 0 / 1, c.aa as above
+cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
+cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+cudaError_t launch_thermal_walls(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
+cudaError_t launch_thermal_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+
 }  // namespace tcp

@@ -49,12 +49,37 @@ cudaError_t by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t 
     }
 }
 
+template <typename real, int QT, bool WALLS>
+cudaError_t thermal_dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
+    switch (2 * c.aa + (c.mode == 1)) {
+    case 0: thermal_only_kernel<real, QT, WALLS, 0, 0><<<c.grid, kBlock, 0, stream>>>(A); break;
+    case 1: thermal_only_kernel<real, QT, WALLS, 1, 0><<<c.grid, kBlock, 0, stream>>>(A); break;
+    case 2: thermal_only_kernel<real, QT, WALLS, 0, 1><<<c.grid, kBlock, 0, stream>>>(A); break;
+    case 3: thermal_only_kernel<real, QT, WALLS, 1, 1><<<c.grid, kBlock, 0, stream>>>(A); break;
+    case 4: thermal_only_kernel<real, QT, WALLS, 0, 2><<<c.grid, kBlock, 0, stream>>>(A); break;
+    default: thermal_only_kernel<real, QT, WALLS, 1, 2><<<c.grid, kBlock, 0, stream>>>(A); break;
+    }
+    return cudaGetLastError();
+}
+template <typename real, bool WALLS>
+cudaError_t thermal_by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
+    switch (c.qt) {
+    case 7: return thermal_dispatch<real, 7, WALLS>(c, A, stream);
+    case 15: return thermal_dispatch<real, 15, WALLS>(c, A, stream);
+    case 19: return thermal_dispatch<real, 19, WALLS>(c, A, stream);
+    case 27: return thermal_dispatch<real, 27, WALLS>(c, A, stream);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
 }  // namespace
 
 #ifdef TCP_WALLS_ONLY
 cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, true>(c, A, stream); }
+cudaError_t launch_thermal_walls(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return thermal_by_stencil<TCP_REAL, true>(c, A, stream); }
 #else
 cudaError_t launch_fused_periodic(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, false>(c, A, stream); }
+cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return thermal_by_stencil<TCP_REAL, false>(c, A, stream); }
 #endif
 
 }  // namespace tcp

@@ -287,6 +287,10 @@ __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const Step
     {
         real g[27];
         pull27<real, WALLS>(A, nb, A.g_in, g);
+        if (WALLS && A.moving) {
+#pragma unroll
+            for (int q = 0; q < 27; ++q) g[q] += wall_velocity_term<real, WALLS>(A, nb, q);
+        }
         collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
 #pragma unroll
         for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
@@ -413,10 +417,19 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         real g[27];
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = stage[(27 + q) * kBlock + tid];
+        if (WALLS && aa != 1 && A.moving) {
+#pragma unroll
+            for (int q = 0; q < 27; ++q) g[q] += wall_velocity_term<real, WALLS>(A, nb, q);
+        }
         if constexpr (MODE != 3) collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
         if (active) {
 #pragma unroll
-            for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.g_out, 27, q, q, wl) = g[q]; }
+            for (int q = 0; q < 27; ++q) {
+                bool wl;
+                real* dst = dst_of(A.g_out, 27, q, q, wl);
+                // AA odd step, link into a moving wall: store what comes back, direction opp(q) with its wall term
+                *dst = (WALLS && wl) ? g[q] + wall_velocity_term<real, WALLS>(A, nb, 26 - q) : g[q];
+            }
             A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
         }
     }
@@ -453,6 +466,63 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
             A.T_out[cell] = Tn;
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// thermal_only_kernel: the thermal LB update alone, with phi and u frozen (temperature
+// pre-initialisation; tcp_relax_temperature).  Same addressing tables as the fused kernel.
+template <typename real, bool WALLS, int AA>
+__device__ __forceinline__ const real* pop_src(const Nbh<WALLS>& nb, const real* base, long long N, int Q, int k, int q27i) {
+    const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
+    if (AA == 1) return base + k * N + nb.idx;
+    int face = 0;
+    const bool bb = WALLS && nb.crossed(-cx, -cy, -cz, face) >= 0;
+    const int plane = (bb != (AA == 2)) ? Q - 1 - k : k;
+    return base + plane * N + (bb ? nb.idx : nb.at(-cx, -cy, -cz));
+}
+template <typename real, bool WALLS, int AA>
+__device__ __forceinline__ real* pop_dst(const Nbh<WALLS>& nb, real* base, long long N, int Q, int k, int q27i, bool& wall_link) {
+    const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
+    wall_link = false;
+    if (AA == 0) return base + k * N + nb.idx;
+    if (AA == 1) return base + (Q - 1 - k) * N + nb.idx;
+    int face = 0;
+    wall_link = WALLS && nb.crossed(cx, cy, cz, face) >= 0;
+    return wall_link ? base + (Q - 1 - k) * N + nb.idx : base + k * N + nb.at(cx, cy, cz);
+}
+
+template <typename real, int QT, bool WALLS, int MODE, int AA>
+__global__ void __launch_bounds__(kBlock) thermal_only_kernel(const StepArgs<real> A) {
+    const int gtid = blockIdx.x * kBlock + threadIdx.x;
+    if (gtid >= A.ncell) return;
+    const long long N = A.ncell;
+    Nbh<WALLS> nb;
+    nb.init(A, gtid);
+    const int cell = nb.idx;
+    real f[QT];
+    static_for<0, QT>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(QT, k);
+        int face = 0;
+        const int ax = AA == 1 ? -1 : nb.crossed(-cx27(q), -cy27(q), -cz27(q), face);
+        const real v = *pop_src<real, WALLS, AA>(nb, A.f_in, N, QT, k, q);
+        f[k] = (WALLS && ax >= 0) ? real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, -cx27(q), -cy27(q), -cz27(q)) - v : v;
+    });
+    const real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
+    const real qT = A.q_src ? A.q_src[cell] : real(0);
+    const real Tn = collide_thermal<real, QT, MODE>(A, f, A.phi_in[cell], u, qT);
+    static_for<0, QT>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(QT, k);
+        bool wl;
+        real* dst = pop_dst<real, WALLS, AA>(nb, A.f_out, N, QT, k, q, wl);
+        real v = f[k];
+        if (WALLS && wl) {
+            int face = 0;
+            const int ax = nb.crossed(cx27(q), cy27(q), cz27(q), face);
+            v = real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, cx27(q), cy27(q), cz27(q)) - v;
+        }
+        *dst = v;
+    });
+    A.T_out[cell] = Tn;
 }
 
 // ---- Runge-Kutta stages of eq. 4 (eqs. 25-26; reading G6) --------------------
@@ -530,7 +600,11 @@ __global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
     }
     equilibrium_plus_half_force27<real>(-real(1.5) * uu, u, u, u, out);                   // eq. 18, p* = 0
 #pragma unroll
-    for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.g_out, 27, q, q, wl) = out[q]; }
+    for (int q = 0; q < 27; ++q) {
+        bool wl;
+        real* dst = dst_of(A.g_out, 27, q, q, wl);
+        *dst = wl ? out[q] + wall_velocity_term<real, true>(A, nb, 26 - q) : out[q];
+    }
     if constexpr (QT > 0) {
         real f[QT];
         thermal_equilibrium<real, QT>(A.T_in[cell], u, f);

@@ -9,8 +9,12 @@ template <typename real, int QT, bool WALLS, int MODE, int AA>
 cudaError_t launch_staged(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
     const size_t smem = (size_t)(54 + QT) * kBlock * sizeof(real);
     auto kern = fused_step_async_kernel<real, QT, WALLS, MODE, AA>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    static bool configured = false;      // once per instantiation (one device per process): saves ~1 us per launch
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
     kern<<<c.grid, kBlock, smem, stream>>>(A);
     return cudaGetLastError();
 }

@@ -12,9 +12,6 @@
 
 #include "tcp_launch.h"
 #include "tcp_rk.cuh"
-#ifdef TCP_EXPERIMENTAL_ROWS
-#include "tcp_rows.cuh"
-#endif
 
 namespace {
 
@@ -115,11 +112,7 @@ struct tcp_sim {
     long long launches;
     cudaEvent_t ev0, ev1;
     bool use_async;          // cp.async staged kernel
-    int bz;                  // z-slab thickness of the cell visiting order
     int aa_next;             // AA streaming: type of the next step (1 even, 2 odd); 0 = two-grid
-    bool use_rows;           // TMA row-segment kernel eligible (x periodic, nx % (16 B / element) == 0, not BGK)
-    int rows_L, rows_threads;
-    size_t rows_smem;
 };
 
 namespace {
@@ -133,7 +126,6 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     const tcp_params& P = s->P;
     const int c = s->cur, o = 1 - s->cur, cT = s->curT, oT = 1 - s->curT;
     A.nx = s->nx; A.ny = s->ny; A.nz = s->nz; A.ncell = (int)s->N;
-    A.bz = s->bz;
     A.aa = s->aa_next;
     for (int a = 0; a < 3; ++a) A.wall[a] = P.bc[a] == TCP_BC_WALLS;
     A.h_in = ptr<real>(s, s->L.h[c]); A.h_out = ptr<real>(s, s->L.h[o]);
@@ -184,29 +176,6 @@ void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
     else tcp::rk_stage_kernel<real, false><<<grid, tcp::kBlock, 0, s->stream>>>(R);
 }
 
-#ifdef TCP_EXPERIMENTAL_ROWS
-template <typename real, bool WALLS>
-int launch_rows(const tcp_sim* s, const tcp::StepArgs<real>& A) {
-    const dim3 grid((unsigned)((s->nx + s->rows_L - 1) / s->rows_L), (unsigned)s->ny, (unsigned)s->nz);
-    const dim3 block((unsigned)s->rows_threads);
-#define TCP_ROWS_LAUNCH(Q)                                                                                         \
-    do {                                                                                                           \
-        auto kern = tcp::fused_step_rows_kernel<real, Q, WALLS>;                                                  \
-        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->rows_smem));           \
-        kern<<<grid, block, s->rows_smem, s->stream>>>(A, s->rows_L);                                             \
-    } while (0)
-    switch (thermal_q(s->P.thermal)) {
-    case 7: TCP_ROWS_LAUNCH(7); break;
-    case 15: TCP_ROWS_LAUNCH(15); break;
-    case 19: TCP_ROWS_LAUNCH(19); break;
-    case 27: TCP_ROWS_LAUNCH(27); break;
-    default: TCP_ROWS_LAUNCH(0); break;
-    }
-#undef TCP_ROWS_LAUNCH
-    return TCP_OK;
-}
-
-#endif
 
 // Runge-Kutta update of T (eqs. 25-26) from T[curT] into T[1 - curT]; phi = the phi to differentiate
 template <typename real>
@@ -278,12 +247,6 @@ int step_once(tcp_sim* s) {
         c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
         c.staged = s->use_async || mode != 0 || c.aa != 0;
         c.grid = grid_for(s->N);
-#ifdef TCP_EXPERIMENTAL_ROWS
-        if (!c.staged && s->use_rows) {
-            int rc = s->walls ? launch_rows<real, true>(s, A) : launch_rows<real, false>(s, A);
-            if (rc) return rc;
-        } else
-#endif
         CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
     }
     s->launches++;
@@ -380,26 +343,10 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
     s->L = make_layout(nx, ny, nz, p);
     s->walls = p->bc[0] == TCP_BC_WALLS || p->bc[1] == TCP_BC_WALLS || p->bc[2] == TCP_BC_WALLS;
     s->owns_memory = own; s->owns_stream = own;
-    {   // kernel choice: the TMA row-segment kernel where its alignment rules hold (tcp_rows.cuh), else the flat one.
-        // TCP_KERNEL=flat / rows overrides (tuning and A/B tests); TCP_ROWS_L sets the segment length.
-        const int es = p->precision == TCP_F64 ? 8 : 4, AH = 16 / es;
+    {   // default: the cp.async staged kernels; TCP_KERNEL=flat selects the register-staged fused kernel and the
+        // flat RK stage kernel for A/B runs (two-grid, default collision mode only; anything else stays staged)
         const char* force = std::getenv("TCP_KERNEL");
-        s->use_rows = p->bc[0] == TCP_BC_PERIODIC && nx % AH == 0 && !p->high_rate_equals_shear && p->s_high == 1.0;
-        s->bz = 1;   // measured at 400^3: slabs of 8 / 16 / 32 planes are 2-3 % SLOWER than plain z order (profiles/r01_notes.md)
-        if (const char* b = std::getenv("TCP_BZ")) { int v = std::atoi(b); if (v >= 1) s->bz = v < nz ? v : nz; }
-        // default: the cp.async staged kernel; TCP_KERNEL=flat (register-staged) / rows (TMA bulk rows) for A/B runs
-        s->use_async = !force || std::strcmp(force, "async") == 0;
-        if (!force || std::strcmp(force, "rows") != 0) s->use_rows = false;
-        if (p->streaming == TCP_STREAM_AA) { s->use_async = true; s->use_rows = false; }   // only the staged kernel knows the AA addressing
-        int cap = 128;
-        if (const char* l = std::getenv("TCP_ROWS_L")) { int v = std::atoi(l); if (v >= AH && v <= cap) cap = v; }
-        const int nseg = (nx + cap - 1) / cap;
-        int L = (nx + nseg - 1) / nseg;
-        L = (L + AH - 1) / AH * AH;
-        s->rows_L = L;
-        s->rows_threads = (L + 31) / 32 * 32;
-        s->rows_smem = (size_t)(54 + thermal_q(p->thermal)) * (L + 2 * AH) * es + 64;
-        if (s->rows_smem > 200 * 1024) s->use_rows = false;
+        s->use_async = !(force && std::strcmp(force, "flat") == 0);
     }
     if (own) {
         void* mem = nullptr;

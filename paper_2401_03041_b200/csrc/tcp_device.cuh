@@ -13,7 +13,6 @@ template <typename real>
 struct StepArgs {
     int nx, ny, nz;
     int ncell;                       // nx*ny*nz < 2^31
-    int bz;                          // z-slab thickness of the visiting order (Nbh::init)
     int aa;                          // streaming: 0 two-grid pull; AA in place: 1 even step, 2 odd step (tcp_step.cuh)
     int wall[3];                     // 1 = WALLS on that axis
     const real* h_in;  real* h_out;  // [27][N]
@@ -46,20 +45,12 @@ struct Nbh {
     int X[3], Y[3], Z[3];            // WALLS: coordinates of the wrapped / mirrored neighbours
     int nx, ny;
 
+    // thread id -> cell: plain x, y, z order (a z-slab visiting order was measured 2-3 % slower, profiles/r01_notes.md)
     template <typename real>
-    // thread id -> cell.  Rows are visited x fastest, then z within a slab of A.bz planes, then y,
-    // then slab: the 3 x 3 rows of phi and T a cell differentiates are then re-read within ~2 bz rows
-    // (a few MB of traffic) instead of a whole z-plane later (169 MB at 400^2 cells per plane, more
-    // than the 126 MB L2, which cost 32 B per cell of halo re-fetch).
-    __device__ __forceinline__ void init(const StepArgs<real>& A, int tid_global) {
-        const int x = tid_global % A.nx;
-        const int r = tid_global / A.nx;            // row number in visiting order
-        const int per_slab = A.ny * A.bz;
-        const int slab = r / per_slab, rem = r - slab * per_slab;
-        const int z0 = slab * A.bz;
-        const int bz = min(A.bz, A.nz - z0);        // last slab may be thinner
-        const int y = rem / bz, zi = rem - y * bz;
-        init_xyz(A, x, y, z0 + zi);
+    __device__ __forceinline__ void init(const StepArgs<real>& A, int cell) {
+        const int x = cell % A.nx;
+        const int t = cell / A.nx;
+        init_xyz(A, x, t % A.ny, t / A.ny);
     }
     template <typename real>
     __device__ __forceinline__ void init_xyz(const StepArgs<real>& A, int x, int y, int z) {

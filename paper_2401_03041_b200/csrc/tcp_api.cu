@@ -112,6 +112,7 @@ struct tcp_sim {
     long long launches;
     cudaEvent_t ev0, ev1;
     bool use_async;          // cp.async staged kernel
+    bool use_pair;           // fp32: two cells per thread, packed arithmetic (x periodic, nx even)
     int aa_next;             // AA streaming: type of the next step (1 even, 2 odd); 0 = two-grid
 };
 
@@ -247,7 +248,15 @@ int step_once(tcp_sim* s) {
         c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
         c.staged = s->use_async || mode != 0 || c.aa != 0;
         c.grid = grid_for(s->N);
-        CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+        if constexpr (sizeof(real) == 4) {
+            if (s->use_pair && c.staged && mode == 0) {
+                CK(s->walls ? tcp::launch_pair_walls(c, A, s->stream) : tcp::launch_pair_periodic(c, A, s->stream));
+            } else {
+                CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+            }
+        } else {
+            CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+        }
     }
     s->launches++;
     rk_update<real>(s, A, A.phi_out);        // phi^{n+1}; u already holds u^{n+1}
@@ -347,6 +356,8 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
         // flat RK stage kernel for A/B runs (two-grid, default collision mode only; anything else stays staged)
         const char* force = std::getenv("TCP_KERNEL");
         s->use_async = !(force && std::strcmp(force, "flat") == 0);
+        // fp32: the packed-pair kernel wherever its layout rules hold; TCP_KERNEL=scalar keeps one cell per thread
+        s->use_pair = p->precision == TCP_F32 && p->bc[0] == TCP_BC_PERIODIC && nx % 2 == 0 && !(force && std::strcmp(force, "scalar") == 0);
     }
     if (own) {
         void* mem = nullptr;

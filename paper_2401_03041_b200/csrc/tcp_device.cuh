@@ -6,6 +6,7 @@
 // same operator is evaluated in closed form).
 #pragma once
 #include "tcp_lattice.cuh"
+#include "tcp_real.cuh"
 
 namespace tcp {
 
@@ -31,6 +32,46 @@ struct StepArgs {
     real s_bulk, s_high, eps;
     int moving;                      // any wall velocity non-zero
     real wall_u[3][2][3];            // wall velocity [axis][face][component] (moving wall, reading S18)
+};
+
+// packed pairs: the arrays are plain float arrays, the scalars are broadcast pairs
+template <>
+struct StepArgs<f32x2> {
+    int nx, ny, nz;
+    int ncell;
+    int aa;
+    int wall[3];
+    const float* h_in;  float* h_out;
+    const float* g_in;  float* g_out;
+    const float* f_in;  float* f_out;
+    const float* phi_in; float* phi_out;
+    const float* T_in;  float* T_out;
+    float* u;
+    const float* q_src;
+    const float* wallT[3][2];
+    f32x2 rho_L, drho, tau_L, dtau;
+    f32x2 xi, w_phi;
+    f32x2 sigma_ref, sigma_T, T_ref;
+    f32x2 kappa_L, dkappa, cp_L, dcp;
+    f32x2 grav[3];
+    f32x2 s_bulk, s_high, eps;
+    int moving;
+    float wall_u[3][2][3];
+    __host__ explicit StepArgs(const StepArgs<float>& A)
+        : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
+          f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src),
+          rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), sigma_ref(A.sigma_ref),
+          sigma_T(A.sigma_T), T_ref(A.T_ref), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
+          s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving) {
+        for (int a = 0; a < 3; ++a) {
+            wall[a] = A.wall[a];
+            grav[a] = f32x2(A.grav[a]);
+            for (int f = 0; f < 2; ++f) {
+                wallT[a][f] = A.wallT[a][f];
+                for (int k = 0; k < 3; ++k) wall_u[a][f][k] = A.wall_u[a][f][k];
+            }
+        }
+    }
 };
 
 // ---------------------------------------------------------------------------------------------

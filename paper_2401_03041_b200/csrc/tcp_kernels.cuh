@@ -16,9 +16,6 @@
 
 namespace tcp {
 
-template <typename real> __device__ __forceinline__ real rsqrt_(real x);
-template <> __device__ __forceinline__ double rsqrt_<double>(double x) { return 1.0 / sqrt(x); }
-template <> __device__ __forceinline__ float rsqrt_<float>(float x) { return 1.0f / sqrtf(x); }
 
 // ---------------------------------------------------------------------------------------------
 // thermal lattice helpers (stencil Q, compact index k)

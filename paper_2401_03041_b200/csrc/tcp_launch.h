@@ -21,6 +21,10 @@ cudaError_t launch_fused_periodic(const FusedCfg& c, const StepArgs<float>& A, c
 cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
 cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
 
+// single precision, two cells per thread, packed arithmetic (tcp_pair.cuh): x periodic and nx even only
+cudaError_t launch_pair_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+cudaError_t launch_pair_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+
 // thermal LB update alone (tcp_relax_temperature); c.mode 0 / 1, c.aa as above
 cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
 cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);

@@ -1,6 +1,9 @@
 // Included by tcp_fused_f64.cu / tcp_fused_f32.cu with TCP_REAL defined.
 #include "tcp_launch.h"
 #include "tcp_step.cuh"
+#ifdef TCP_PAIR
+#include "tcp_pair.cuh"
+#endif
 
 namespace tcp {
 namespace {
@@ -76,7 +79,52 @@ cudaError_t thermal_by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaS
     }
 }
 
+#ifdef TCP_PAIR
+// packed-pair single-precision kernels (tcp_pair.cuh)
+template <int QT, bool WALLS, int MODE, int AA>
+cudaError_t launch_pair(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_t stream) {
+    const size_t smem = (size_t)(54 + QT) * kBlock * sizeof(float2);
+    auto kern = fused_step_pair_kernel<QT, WALLS, MODE, AA>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const unsigned grid = (unsigned)(((A.ncell >> 1) + kBlock - 1) / kBlock);
+    kern<<<grid, kBlock, smem, stream>>>(A);
+    return cudaGetLastError();
+}
+template <int QT, bool WALLS>
+cudaError_t pair_dispatch(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_t stream) {
+    switch (c.aa) {   // default collision mode only (BGK and general rates run the scalar kernels)
+    case 0: return launch_pair<QT, WALLS, 0, 0>(c, A, stream);
+    case 1: return launch_pair<QT, WALLS, 0, 1>(c, A, stream);
+    default: return launch_pair<QT, WALLS, 0, 2>(c, A, stream);
+    }
+}
+template <bool WALLS>
+cudaError_t pair_by_stencil(const FusedCfg& c, const StepArgs<float>& Af, cudaStream_t stream) {
+    const StepArgs<f32x2> A(Af);
+    switch (c.qt) {
+    case 7: return pair_dispatch<7, WALLS>(c, A, stream);
+    case 15: return pair_dispatch<15, WALLS>(c, A, stream);
+    case 19: return pair_dispatch<19, WALLS>(c, A, stream);
+    case 27: return pair_dispatch<27, WALLS>(c, A, stream);
+    default: return pair_dispatch<0, WALLS>(c, A, stream);
+    }
+}
+#endif
+
 }  // namespace
+
+#ifdef TCP_PAIR
+#ifdef TCP_WALLS_ONLY
+cudaError_t launch_pair_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream) { return pair_by_stencil<true>(c, A, stream); }
+#else
+cudaError_t launch_pair_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream) { return pair_by_stencil<false>(c, A, stream); }
+#endif
+#endif
 
 #ifdef TCP_WALLS_ONLY
 cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, true>(c, A, stream); }

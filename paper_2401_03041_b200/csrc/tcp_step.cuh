@@ -22,19 +22,19 @@ constexpr int kBlock = TCP_BLOCK;
 // what is left is one unbiased rounding per cell and step.  In fp64 the bias is ~1e-17 per step
 // and the arithmetic is left as derived.
 template <typename real>
-__device__ __forceinline__ double exact_sum27(const real a[27]) {
-    double s = 0.0;
+__device__ __forceinline__ wide_t<real> exact_sum27(const real a[27]) {
+    wide_t<real> s = wide_zero<real>();
 #pragma unroll
-    for (int q = 0; q < 27; ++q) s += (double)a[q];
+    for (int q = 0; q < 27; ++q) s += widen(a[q]);
     return s;
 }
 template <typename real>
-__device__ __forceinline__ void conserve_zeroth27(real a[27], double s) {
-    if constexpr (sizeof(real) == 4) {
+__device__ __forceinline__ void conserve_zeroth27(real a[27], wide_t<real> s) {
+    if constexpr (real_traits<real>::single) {
 #pragma unroll
         for (int q = 0; q < 27; ++q)
-            if (q != 13) s -= (double)a[q];
-        a[13] = (real)s;
+            if (q != 13) s -= widen(a[q]);
+        a[13] = narrow<real>(s);
     }
 }
 
@@ -76,9 +76,9 @@ __device__ __forceinline__ void central_transform27(real X[27], const real u[3])
 template <typename real, int MODE>
 __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27], const real G[3], real phi_c, const real un[3]) {
     const Mom2<real> M = moments27<real, false>(h);
-    double phin_exact = 0.0;
-    if constexpr (sizeof(real) == 4) phin_exact = exact_sum27<real>(h);
-    const real phin = sizeof(real) == 4 ? (real)phin_exact : M.m0;
+    wide_t<real> phin_exact = wide_zero<real>();
+    real phin = M.m0;
+    if constexpr (real_traits<real>::single) { phin_exact = exact_sum27<real>(h); phin = narrow<real>(phin_exact); }
     // a = c_s^2 [4 phi (1 - phi) / xi] n,  n = G / sqrt(G.G + eps)   (eq. 15, readings S7, S8)
     const real inv = rsqrt_<real>(G[0] * G[0] + G[1] * G[1] + G[2] * G[2] + A.eps);
     const real mag = real(4.0 / 3.0) * phi_c * (real(1) - phi_c) / A.xi * inv;
@@ -119,9 +119,9 @@ template <typename real, int MODE>
 __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27], real phi_c, const real G[3], real lapPhi,
                                               real T_c, const real Th[3], real u[3]) {
     const Mom2<real> M = moments27<real, true>(g);
-    double ps_exact = 0.0;
-    if constexpr (sizeof(real) == 4) ps_exact = exact_sum27<real>(g);
-    const real ps = sizeof(real) == 4 ? (real)ps_exact : M.m0;   // p* (eq. 17)
+    wide_t<real> ps_exact = wide_zero<real>();
+    real ps = M.m0;                                         // p* (eq. 17)
+    if constexpr (real_traits<real>::single) { ps_exact = exact_sum27<real>(g); ps = narrow<real>(ps_exact); }
     const real j[3] = {M.mx, M.my, M.mz};
     const real rho = A.rho_L + phi_c * A.drho;              // eq. 14
     const real tau = A.tau_L + phi_c * A.dtau;              // eq. 22
@@ -221,16 +221,16 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
 template <typename real, int Q, int MODE>
 __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[Q], real phi_new, const real u[3], real qT) {
     real Tn = real(0), j[3] = {real(0), real(0), real(0)};
-    double Tn_exact = 0.0;
+    wide_t<real> Tn_exact = wide_zero<real>();
     static_for<0, Q>([&](auto K) {
         constexpr int k = decltype(K)::value, q = q_of(Q, k);
-        if constexpr (sizeof(real) == 4) Tn_exact += (double)f[k]; else
+        if constexpr (real_traits<real>::single) Tn_exact += widen(f[k]); else
         Tn += f[k];                                          // eq. 28
         if constexpr (cx27(q) != 0) j[0] += real(cx27(q)) * f[k];
         if constexpr (cy27(q) != 0) j[1] += real(cy27(q)) * f[k];
         if constexpr (cz27(q) != 0) j[2] += real(cz27(q)) * f[k];
     });
-    if constexpr (sizeof(real) == 4) Tn = (real)Tn_exact;
+    if constexpr (real_traits<real>::single) Tn = narrow<real>(Tn_exact);
     const real kap = A.kappa_L + phi_new * A.dkappa;         // eq. 23 (G5)
     const real w = real(1) / (real(0.5) + real(3) * kap);    // eq. 29 read as a rate (G4)
     real out[Q];
@@ -248,10 +248,10 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
             add_first_order_thermal<real, Q>(m, u, out);
         }
     }
-    if constexpr (sizeof(real) == 4) {   // see conserve_zeroth27
-        double rest = Tn_exact;
-        static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; if constexpr (k != Q / 2) rest -= (double)out[k]; });
-        out[Q / 2] = (real)rest;
+    if constexpr (real_traits<real>::single) {   // see conserve_zeroth27
+        wide_t<real> rest = Tn_exact;
+        static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; if constexpr (k != Q / 2) rest -= widen(out[k]); });
+        out[Q / 2] = narrow<real>(rest);
     }
     static_for<0, Q>([&](auto K) {
         constexpr int k = decltype(K)::value, q = q_of(Q, k);

@@ -110,3 +110,33 @@ def test_full_size_sampled_parity_400_cubed_d3q7():
 
 def test_full_size_sampled_parity_rk4_256():
     assert _sampled_parity(256, "rk4", steps=2, samples=8, half=8) <= 1e-10
+
+
+@pytest.mark.parametrize("streaming", ["two_grid", "aa"])
+@pytest.mark.parametrize("thermal", ["lb_d3q7", "lb_d3q15", "lb_d3q27", "rk2"])
+def test_fp32_packed_pair_kernel_against_scalar_kernel_and_oracle(thermal, streaming, monkeypatch):
+    """fp32 runs two x-adjacent cells per thread with packed FFMA2 arithmetic where x is periodic and nx even
+    (tcp_pair.cuh); TCP_KERNEL=scalar keeps one cell per thread.  Both must meet the fp32 bar against the
+    oracle, with y / z walls, a wall-temperature plane, moving walls and odd / even AA step counts."""
+    wl = W.thermal_tweezer(nx=36, ny=20, nz=18, thermal=thermal, R=5.0, offset=7.0, A=2.0, s=4.0)
+    wu = [[[0.0] * 3 for _ in range(2)] for _ in range(3)]
+    wu[2][1] = [1e-3, -5e-4, 0.0]
+    extra = dict(wall_u=wu, streaming=streaming)
+    for steps in (40, 41):
+        want = run_oracle(wl, steps, extra=extra)
+        monkeypatch.delenv("TCP_KERNEL", raising=False)
+        got_pair, _ = run_gpu(wl, steps, extra=extra, precision="f32")
+        monkeypatch.setenv("TCP_KERNEL", "scalar")
+        got_scalar, _ = run_gpu(wl, steps, extra=extra, precision="f32")
+        monkeypatch.delenv("TCP_KERNEL", raising=False)
+        assert_parity_f32(got_pair, want)
+        assert_parity_f32(got_scalar, want)
+        # the two fp32 kernels differ only by round-off order
+        assert np.abs(got_pair[0].astype(np.float64) - got_scalar[0]).max() < 2e-6
+
+
+def test_fp32_odd_nx_falls_back_to_the_scalar_kernel():
+    wl = W.perf_box(23, thermal="lb_d3q19", ny=14, nz=12, r_min=3.0, r_max=4.0, seed=6)
+    want = run_oracle(wl, 60)
+    got, _ = run_gpu(wl, 60, precision="f32")
+    assert_parity_f32(got, want)

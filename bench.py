@@ -308,6 +308,65 @@ def run_sweep(args):
             torch.cuda.empty_cache()
 
 
+def run_slabs(args):
+    """The same box cut into z-slabs with ghost planes (tcp_step_begin / tcp_step_end).
+    One GPU: `--slabs K` runs K slabs of the size^3 box in this process (the transfer is a device copy), which
+    measures what the split step and the gather / scatter cost.  N > 1 ranks with `--decompose`: one slab per
+    rank of a size x size x (size * N) box (weak scaling), messages over torch.distributed point-to-point.
+    Device-resident timing only; not the driver's line."""
+    from paper_2401_03041_b200 import binding as B
+    from paper_2401_03041_b200.slab import LocalSlabs, RankSlab
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    n, thermal, prec = args.size, args.thermal, args.precision
+    tdt = torch.float64 if prec == "f64" else torch.float32
+    wl = W.perf_box(n, thermal=thermal, device="cuda", seed=20240103 + n + rank)
+    params = dict(wl.params, precision=prec)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        box = RankSlab(n, n, n * world, params)
+        s = box.slab
+        ext = lambda a: box.fill_ghosts(torch.cat([a[:1]] * s.lo + [a] + [a[-1:]] * s.hi).to(tdt).contiguous())
+        s.init_fields(ext(wl.phi), None, ext(wl.T))
+        launches = lambda: s.sim.launches
+        msg = B.tcp_halo_bytes(s.sim._h)
+        desc = f"one z-slab of {n}x{n}x{n} per rank of a {n}x{n}x{n * world} periodic box, NCCL point-to-point"
+    else:
+        box = LocalSlabs(n, n, n, args.slabs, params)
+        box.init_fields(wl.phi.to(tdt), None, wl.T.to(tdt))
+        launches = lambda: box.launches
+        msg = B.tcp_halo_bytes(box.slabs[0].sim._h)
+        desc = f"{n}^3 periodic box in {args.slabs} z-slabs on one GPU, messages by device copy"
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    box.step(args.warmup)
+    barrier()
+    l0 = launches()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    box.step(args.steps)
+    ev1.record()
+    barrier()
+    ms = max_over_ranks(ev0.elapsed_time(ev1), dist)
+    if rank == 0:
+        print(json.dumps({"slabs": True, "metric": METRIC, "value": aggregate_mlups(wl.cells, args.steps, world, ms), "unit": "MLUPS",
+                          "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "dtype": prec,
+                          "scaling": "weak", "config": {"workload": desc, "thermal": thermal, "message_bytes_per_face": msg},
+                          "gpu_launches": launches() - l0}), flush=True)
+    box.close()
+    if dist:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -323,10 +382,14 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="per-variant / per-size table (configs[4]); one JSON line each")
     ap.add_argument("--sweep-sizes", default="", help="e.g. 256:f64,512:f32")
+    ap.add_argument("--slabs", type=int, default=0, help="one GPU: run the box as this many z-slabs with ghost planes")
+    ap.add_argument("--decompose", action="store_true", help="N > 1: one z-slab per rank of one box instead of replicas")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: W >= 3
-    if args.sweep:
+    if args.slabs > 1 or args.decompose:
+        run_slabs(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -100,6 +100,33 @@ int tcp_step(tcp_sim *s, int nsteps);
  * be even.  Errors: TCP_ESTATE, TCP_EINVAL, TCP_ECUDA. */
 int tcp_relax_temperature(tcp_sim *s, int nsteps);
 
+/* ---- block decomposition along z ("the domain is partitioned into blocks ... ghost layers";
+ * Algorithm 1 updates the cells next to a block face first and sends their populations while the interior is
+ * updated).  A slab is an ordinary simulation whose z-plane 0 (`lo`) and / or z-plane nz-1 (`hi`) is a GHOST
+ * plane: it holds a copy of the neighbouring slab's boundary plane, is never updated by this simulation, and
+ * takes the place of the periodic wrap / wall of bc[2] on that face (a face without ghost plane keeps bc[2]).
+ * Arrays passed to tcp_init_fields / tcp_set_heat_source / returned by tcp_read_fields include the ghost
+ * planes (initial phi, T there = the neighbour's values; p is undefined there); wall-temperature planes of the
+ * x and y walls include the ghost rows.  Two-grid streaming and a thermal LB only (TCP_EUNSUPPORTED otherwise).
+ *
+ * One message per face and step: [9 h~ planes][9 g~ planes][1, 5, 5 or 9 f~ planes][phi][T], nx*ny values each,
+ * = tcp_halo_bytes.  `send_*` / `recv_*` are caller-owned DEVICE buffers of that size (NULL for a face without
+ * ghost plane); `comm_stream` is the caller's cudaStream_t on which the library packs and unpacks and on which
+ * the caller must enqueue the transfer send_hi -> upper neighbour's recv_lo, send_lo -> lower neighbour's
+ * recv_hi between tcp_step_begin and tcp_step_end.  lo = hi = 0 turns the slab back into a plain box. */
+int tcp_set_halo(tcp_sim *s, int lo, int hi, void *comm_stream, void *send_lo, void *send_hi, void *recv_lo,
+                 void *recv_hi);
+int tcp_halo_bytes(const tcp_sim *s, size_t *bytes);
+
+/* One time step of a slab, in two calls.  tcp_step_begin: the fused step on the plane(s) next to a ghost plane
+ * (simulation's stream), then -- on comm_stream, as soon as those are done -- the gather of the new boundary
+ * populations into send_lo / send_hi, and on the simulation's stream the fused step on the interior planes.
+ * tcp_step_end: scatter recv_lo / recv_hi into the ghost planes of the new time level (comm_stream, i.e. after
+ * the transfer the caller enqueued there); the simulation's stream then waits for it.  Both asynchronous.
+ * tcp_step returns TCP_ESTATE on a slab; these return TCP_ESTATE on a plain box or when called out of order. */
+int tcp_step_begin(tcp_sim *s);
+int tcp_step_end(tcp_sim *s);
+
 /* Copy out phi, u, p = c_s^2 rho(phi) sum_i g~_i, T; any pointer may be NULL.
  * Synchronises the stream. */
 int tcp_read_fields(tcp_sim *s, void *phi, void *u, void *p, void *T);

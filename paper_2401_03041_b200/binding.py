@@ -80,7 +80,8 @@ def make_params(d: dict) -> tcp_params:
 
 EXPORTS = ["tcp_workspace_bytes", "tcp_create", "tcp_create_in", "tcp_init_fields", "tcp_set_wall_temperature",
            "tcp_set_heat_source", "tcp_step", "tcp_relax_temperature", "tcp_read_fields", "tcp_synchronize", "tcp_launch_count",
-           "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_destroy", "tcp_last_error"]
+           "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_destroy", "tcp_last_error",
+           "tcp_set_halo", "tcp_halo_bytes", "tcp_step_begin", "tcp_step_end"]
 
 _lib = None
 
@@ -111,6 +112,10 @@ def lib():
         L.tcp_last_step_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.tcp_pattern_copy_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
         L.tcp_destroy.argtypes = [vp]
+        L.tcp_set_halo.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp]
+        L.tcp_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+        L.tcp_step_begin.argtypes = [vp]
+        L.tcp_step_end.argtypes = [vp]
         L.tcp_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -202,6 +207,25 @@ def tcp_pattern_copy_ms(sim, nlaunches=10) -> float:
     ms = C.c_float()
     _check(lib().tcp_pattern_copy_ms(sim, int(nlaunches), C.byref(ms)))
     return float(ms.value)
+
+
+def tcp_set_halo(sim, lo, hi, comm_stream: "torch.cuda.Stream | None", send_lo=None, send_hi=None, recv_lo=None, recv_hi=None):
+    sp = C.c_void_p(comm_stream.cuda_stream if comm_stream is not None else 0)
+    _check(lib().tcp_set_halo(sim, int(lo), int(hi), sp, _ptr(send_lo), _ptr(send_hi), _ptr(recv_lo), _ptr(recv_hi)))
+
+
+def tcp_halo_bytes(sim) -> int:
+    n = C.c_size_t()
+    _check(lib().tcp_halo_bytes(sim, C.byref(n)))
+    return n.value
+
+
+def tcp_step_begin(sim):
+    _check(lib().tcp_step_begin(sim))
+
+
+def tcp_step_end(sim):
+    _check(lib().tcp_step_end(sim))
 
 
 def tcp_destroy(sim):

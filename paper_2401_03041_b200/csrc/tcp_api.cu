@@ -10,6 +10,7 @@
 #include "../../include/tcp.h"
 #include <cstdlib>
 
+#include "tcp_halo.cuh"
 #include "tcp_launch.h"
 #include "tcp_rk.cuh"
 
@@ -114,6 +115,13 @@ struct tcp_sim {
     bool use_async;          // cp.async staged kernel
     bool use_pair;           // fp32: two cells per thread, packed arithmetic (x periodic, nx even)
     int aa_next;             // AA streaming: type of the next step (1 even, 2 odd); 0 = two-grid
+    // z-slab of a decomposed box (tcp_set_halo): plane 0 / nz-1 is a ghost plane filled from a neighbour
+    bool halo[2];
+    bool in_step;            // between tcp_step_begin and tcp_step_end
+    cudaStream_t comm;       // caller's stream for pack / exchange / unpack
+    void* send[2];           // caller's device buffers, one message each
+    void* recv[2];
+    cudaEvent_t ev_bnd, ev_comm;
 };
 
 namespace {
@@ -127,6 +135,7 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     const tcp_params& P = s->P;
     const int c = s->cur, o = 1 - s->cur, cT = s->curT, oT = 1 - s->curT;
     A.nx = s->nx; A.ny = s->ny; A.nz = s->nz; A.ncell = (int)s->N;
+    A.cell0 = 0; A.cell1 = (int)s->N;
     A.aa = s->aa_next;
     for (int a = 0; a < 3; ++a) A.wall[a] = P.bc[a] == TCP_BC_WALLS;
     A.h_in = ptr<real>(s, s->L.h[c]); A.h_out = ptr<real>(s, s->L.h[o]);
@@ -236,33 +245,127 @@ int relax_t(tcp_sim* s, int nsteps) {
     return TCP_OK;
 }
 
+// the fused phase + hydro (+ thermal LB) kernel on the cells [A.cell0, A.cell1)
+template <typename real>
+int launch_fused(tcp_sim* s, const tcp::StepArgs<real>& A) {
+    // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
+    const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
+    tcp::FusedCfg c;
+    c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
+    c.staged = s->use_async || mode != 0 || c.aa != 0;
+    c.grid = grid_for((size_t)(A.cell1 - A.cell0));
+    if constexpr (sizeof(real) == 4) {
+        if (s->use_pair && c.staged && mode == 0) {
+            CK(s->walls ? tcp::launch_pair_walls(c, A, s->stream) : tcp::launch_pair_periodic(c, A, s->stream));
+        } else {
+            CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+        }
+    } else {
+        CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+    }
+    s->launches++;
+    return TCP_OK;
+}
+
 // one time step: Algorithm 1 (thermal LB, one fused kernel) or Algorithm 2 (fused phase+hydro
 // kernel, then the Runge-Kutta stages)
 template <typename real>
 int step_once(tcp_sim* s) {
     tcp::StepArgs<real> A = make_args<real>(s);
-    // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
-    const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
-    {
-        tcp::FusedCfg c;
-        c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
-        c.staged = s->use_async || mode != 0 || c.aa != 0;
-        c.grid = grid_for(s->N);
-        if constexpr (sizeof(real) == 4) {
-            if (s->use_pair && c.staged && mode == 0) {
-                CK(s->walls ? tcp::launch_pair_walls(c, A, s->stream) : tcp::launch_pair_periodic(c, A, s->stream));
-            } else {
-                CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
-            }
-        } else {
-            CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
-        }
-    }
-    s->launches++;
+    int rc = launch_fused<real>(s, A);
+    if (rc) return rc;
     rk_update<real>(s, A, A.phi_out);        // phi^{n+1}; u already holds u^{n+1}
     s->cur = 1 - s->cur;
     s->curT = 1 - s->curT;
     if (s->aa_next) s->aa_next = 3 - s->aa_next;
+    return TCP_OK;
+}
+
+// ---- z-slab with ghost planes (tcp_set_halo): Algorithm 1's order -- boundary cells first, their
+// populations on the way to the neighbour while the interior is updated -----------------
+
+// message travelling in direction dir (+1 up, -1 down): [h~ c_z=dir][g~ c_z=dir][f~ c_z=dir][phi][T], one
+// z-plane each; `gather` copies plane z of the grid into the message, otherwise the message into plane z
+template <typename real>
+void halo_planes(const tcp_sim* s, tcp::HaloCopy& C, int dir, int z, int grid, int gridT, void* message, bool gather) {
+    const size_t P = (size_t)s->nx * s->ny, N = s->N;
+    real* msg = static_cast<real*>(message);
+    int m = 0;
+    auto add = [&](real* plane) {
+        real* in_msg = msg + (size_t)m++ * P;
+        C.src[C.nplanes] = gather ? plane : in_msg;
+        C.dst[C.nplanes] = gather ? in_msg : plane;
+        C.nplanes++;
+    };
+    for (int q = 0; q < 27; ++q)
+        if (tcp::cz27(q) == dir) add(ptr<real>(s, s->L.h[grid]) + q * N + (size_t)z * P);
+    for (int q = 0; q < 27; ++q)
+        if (tcp::cz27(q) == dir) add(ptr<real>(s, s->L.g[grid]) + q * N + (size_t)z * P);
+    const int QT = thermal_q(s->P.thermal);
+    for (int k = 0; k < QT; ++k)
+        if (tcp::cz27(tcp::q_of(QT, k)) == dir) add(ptr<real>(s, s->L.f[gridT]) + k * N + (size_t)z * P);
+    add(ptr<real>(s, s->L.phi[grid]) + (size_t)z * P);
+    add(ptr<real>(s, s->L.T[gridT]) + (size_t)z * P);
+}
+
+template <typename real>
+int halo_copy(tcp_sim* s, const tcp::HaloCopy& C) {
+    if (C.nplanes == 0) return TCP_OK;
+    const dim3 grid((unsigned)((C.plane_cells + 255) / 256), (unsigned)C.nplanes);
+    tcp::halo_copy_kernel<real><<<grid, 256, 0, s->comm>>>(C);
+    s->launches++;
+    CK(cudaGetLastError());
+    return TCP_OK;
+}
+
+template <typename real>
+int step_begin_t(tcp_sim* s) {
+    const int P = s->nx * s->ny;
+    const int zlo = s->halo[0] ? 1 : 0, zhi = s->nz - 1 - (s->halo[1] ? 1 : 0);   // first / last plane this slab owns
+    tcp::StepArgs<real> A = make_args<real>(s);
+    CK(cudaEventRecord(s->ev0, s->stream));
+    auto planes = [&](int z0, int z1) {       // update the planes z0..z1
+        if (z1 < z0) return (int)TCP_OK;
+        A.cell0 = z0 * P; A.cell1 = (z1 + 1) * P;
+        return launch_fused<real>(s, A);
+    };
+    int rc = TCP_OK;
+    if (s->halo[0]) rc = planes(zlo, zlo);
+    if (!rc && s->halo[1] && !(s->halo[0] && zhi == zlo)) rc = planes(zhi, zhi);
+    if (rc) return rc;
+    CK(cudaEventRecord(s->ev_bnd, s->stream));
+    CK(cudaStreamWaitEvent(s->comm, s->ev_bnd, 0));
+    tcp::HaloCopy C;
+    std::memset(&C, 0, sizeof C);
+    C.plane_cells = P;
+    const int o = 1 - s->cur, oT = 1 - s->curT;                                    // the grids this step writes
+    if (s->halo[0]) halo_planes<real>(s, C, -1, zlo, o, oT, s->send[0], true);
+    if (s->halo[1]) halo_planes<real>(s, C, +1, zhi, o, oT, s->send[1], true);
+    rc = halo_copy<real>(s, C);
+    if (rc) return rc;
+    rc = planes(zlo + (s->halo[0] ? 1 : 0), zhi - (s->halo[1] ? 1 : 0));
+    if (rc) return rc;
+    s->in_step = true;
+    return TCP_OK;
+}
+
+template <typename real>
+int step_end_t(tcp_sim* s) {
+    tcp::HaloCopy C;
+    std::memset(&C, 0, sizeof C);
+    C.plane_cells = s->nx * s->ny;
+    const int o = 1 - s->cur, oT = 1 - s->curT;
+    if (s->halo[0]) halo_planes<real>(s, C, +1, 0, o, oT, s->recv[0], false);          // from below, moving up
+    if (s->halo[1]) halo_planes<real>(s, C, -1, s->nz - 1, o, oT, s->recv[1], false);  // from above, moving down
+    int rc = halo_copy<real>(s, C);
+    if (rc) return rc;
+    CK(cudaEventRecord(s->ev_comm, s->comm));
+    CK(cudaStreamWaitEvent(s->stream, s->ev_comm, 0));
+    CK(cudaEventRecord(s->ev1, s->stream));
+    s->cur = 1 - s->cur;
+    s->curT = 1 - s->curT;
+    s->in_step = false;
+    s->stepped = true;
     return TCP_OK;
 }
 
@@ -373,7 +476,9 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
         s->base = static_cast<char*>(workspace);
         s->stream = static_cast<cudaStream_t>(stream);
     }
-    if (cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess) {
+    if (cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess ||
+        cudaEventCreateWithFlags(&s->ev_bnd, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&s->ev_comm, cudaEventDisableTiming) != cudaSuccess) {
         tcp_destroy(s);
         return fail(TCP_ECUDA, "cudaEventCreate failed");
     }
@@ -411,8 +516,11 @@ int tcp_create_in(int nx, int ny, int nz, const tcp_params* p, void* dev_workspa
 int tcp_destroy(tcp_sim* s) {
     if (!s) return TCP_OK;
     cudaStreamSynchronize(s->stream);
+    if (s->halo[0] || s->halo[1]) cudaStreamSynchronize(s->comm);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
+    if (s->ev_bnd) cudaEventDestroy(s->ev_bnd);
+    if (s->ev_comm) cudaEventDestroy(s->ev_comm);
     if (s->owns_stream && s->stream) cudaStreamDestroy(s->stream);
     if (s->owns_memory && s->base) cudaFree(s->base);
     delete s;
@@ -422,6 +530,7 @@ int tcp_destroy(tcp_sim* s) {
 int tcp_init_fields(tcp_sim* s, const void* phi, const void* u, const void* T) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
     if (!phi) return fail(TCP_EINVAL, "phi is required");
+    if (s->in_step) return fail(TCP_ESTATE, "tcp_init_fields between tcp_step_begin and tcp_step_end");
     return s->P.precision == TCP_F64 ? init_fields_t<double>(s, phi, u, T) : init_fields_t<float>(s, phi, u, T);
 }
 
@@ -446,6 +555,7 @@ int tcp_step(tcp_sim* s, int nsteps) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
     if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
     if (nsteps < 0) return fail(TCP_EINVAL, "nsteps must be >= 0");
+    if (s->halo[0] || s->halo[1]) return fail(TCP_ESTATE, "a slab with ghost planes steps with tcp_step_begin / tcp_step_end");
     CK(cudaEventRecord(s->ev0, s->stream));
     for (int n = 0; n < nsteps; ++n) {
         int rc = s->P.precision == TCP_F64 ? step_once<double>(s) : step_once<float>(s);
@@ -462,6 +572,7 @@ int tcp_relax_temperature(tcp_sim* s, int nsteps) {
     if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
     if (nsteps < 0) return fail(TCP_EINVAL, "nsteps must be >= 0");
     const bool lb = thermal_q(s->P.thermal) != 0;
+    if (s->halo[0] || s->halo[1]) return fail(TCP_EUNSUPPORTED, "tcp_relax_temperature: not on a slab with ghost planes");
     if (lb && s->P.streaming == TCP_STREAM_AA && (nsteps & 1))
         return fail(TCP_EINVAL, "AA streaming: the thermal populations must keep the parity of h and g, so nsteps must be even");
     return s->P.precision == TCP_F64 ? relax_t<double>(s, nsteps) : relax_t<float>(s, nsteps);
@@ -482,11 +593,50 @@ int tcp_synchronize(tcp_sim* s) {
 
 long long tcp_launch_count(const tcp_sim* s) { return s ? s->launches : 0; }
 
+int tcp_halo_bytes(const tcp_sim* s, size_t* bytes) {
+    if (!s || !bytes) return fail(TCP_EINVAL, "NULL argument");
+    const int QT = thermal_q(s->P.thermal);
+    const size_t planes = 9 + 9 + (size_t)tcp::halo_crossing(QT, 1) + 2;
+    *bytes = planes * s->nx * s->ny * (s->P.precision == TCP_F64 ? 8 : 4);
+    return TCP_OK;
+}
+
+int tcp_set_halo(tcp_sim* s, int lo, int hi, void* comm_stream, void* send_lo, void* send_hi, void* recv_lo, void* recv_hi) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (s->in_step) return fail(TCP_ESTATE, "tcp_set_halo between tcp_step_begin and tcp_step_end");
+    lo = lo != 0; hi = hi != 0;
+    if (lo || hi) {
+        if (s->P.streaming != TCP_STREAM_TWO_GRID) return fail(TCP_EUNSUPPORTED, "ghost planes: two-grid streaming only");
+        if (thermal_q(s->P.thermal) == 0) return fail(TCP_EUNSUPPORTED, "ghost planes: thermal LB only (the Runge-Kutta stages would need an exchange per stage)");
+        if (s->nz - lo - hi < 1) return fail(TCP_EINVAL, "a slab needs at least one plane of its own between its ghost planes");
+        if ((lo && (!send_lo || !recv_lo)) || (hi && (!send_hi || !recv_hi))) return fail(TCP_EINVAL, "a face with a ghost plane needs a send and a receive buffer");
+    }
+    s->halo[0] = lo; s->halo[1] = hi;
+    s->comm = static_cast<cudaStream_t>(comm_stream);
+    s->send[0] = send_lo; s->send[1] = send_hi; s->recv[0] = recv_lo; s->recv[1] = recv_hi;
+    return TCP_OK;
+}
+
+int tcp_step_begin(tcp_sim* s) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
+    if (!s->halo[0] && !s->halo[1]) return fail(TCP_ESTATE, "tcp_step_begin: no ghost planes (tcp_set_halo); use tcp_step");
+    if (s->in_step) return fail(TCP_ESTATE, "tcp_step_begin called twice without tcp_step_end");
+    return s->P.precision == TCP_F64 ? step_begin_t<double>(s) : step_begin_t<float>(s);
+}
+
+int tcp_step_end(tcp_sim* s) {
+    if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    if (!s->in_step) return fail(TCP_ESTATE, "tcp_step_end without tcp_step_begin");
+    return s->P.precision == TCP_F64 ? step_end_t<double>(s) : step_end_t<float>(s);
+}
+
 int tcp_pattern_copy_ms(tcp_sim* s, int nlaunches, float* ms) {
     if (!s || !ms) return fail(TCP_EINVAL, "NULL argument");
     if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
     if (nlaunches < 1) return fail(TCP_EINVAL, "nlaunches must be >= 1");
-    if (s->walls || s->P.streaming != TCP_STREAM_TWO_GRID) return fail(TCP_EUNSUPPORTED, "pattern copy: periodic two-grid simulations only");
+    if (s->walls || s->P.streaming != TCP_STREAM_TWO_GRID || s->halo[0] || s->halo[1])
+        return fail(TCP_EUNSUPPORTED, "pattern copy: periodic two-grid simulations without ghost planes only");
     tcp::FusedCfg c;
     c.qt = thermal_q(s->P.thermal); c.walls = false; c.mode = 3; c.aa = 0; c.staged = true; c.grid = grid_for(s->N);
     CK(cudaEventRecord(s->ev0, s->stream));

@@ -14,6 +14,8 @@ template <typename real>
 struct StepArgs {
     int nx, ny, nz;
     int ncell;                       // nx*ny*nz < 2^31
+    int cell0, cell1;                // cells [cell0, cell1) are updated by this launch (the whole box, or the
+                                     // boundary planes / the interior of a slab with ghost planes, tcp_step_begin)
     int aa;                          // streaming: 0 two-grid pull; AA in place: 1 even step, 2 odd step (tcp_step.cuh)
     int wall[3];                     // 1 = WALLS on that axis
     const real* h_in;  real* h_out;  // [27][N]
@@ -39,6 +41,7 @@ template <>
 struct StepArgs<f32x2> {
     int nx, ny, nz;
     int ncell;
+    int cell0, cell1;
     int aa;
     int wall[3];
     const float* h_in;  float* h_out;
@@ -58,7 +61,7 @@ struct StepArgs<f32x2> {
     int moving;
     float wall_u[3][2][3];
     __host__ explicit StepArgs(const StepArgs<float>& A)
-        : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
+        : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), cell0(A.cell0), cell1(A.cell1), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
           f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src),
           rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), sigma_ref(A.sigma_ref),
           sigma_T(A.sigma_T), T_ref(A.T_ref), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),

@@ -91,7 +91,7 @@ cudaError_t launch_pair(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    const unsigned grid = (unsigned)(((A.ncell >> 1) + kBlock - 1) / kBlock);
+    const unsigned grid = (unsigned)((((A.cell1 - A.cell0) >> 1) + kBlock - 1) / kBlock);
     kern<<<grid, kBlock, smem, stream>>>(A);
     return cudaGetLastError();
 }

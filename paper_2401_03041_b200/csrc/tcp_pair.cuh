@@ -133,8 +133,8 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair
     using real = f32x2;
     extern __shared__ __align__(16) unsigned char smem_raw_pair[];
     float2* stage = reinterpret_cast<float2*>(smem_raw_pair) + threadIdx.x;     // [54 + QT][kBlock], this thread's column
-    const int npairs = A.ncell >> 1;
-    const int gp = blockIdx.x * kBlock + threadIdx.x;
+    const int npairs = A.cell1 >> 1;                        // cell0, cell1 are even (whole rows of an even nx)
+    const int gp = (A.cell0 >> 1) + blockIdx.x * kBlock + threadIdx.x;
     const bool active = gp < npairs;
     const long long N = A.ncell;
     NbhPair<WALLS> nb;

@@ -263,8 +263,8 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
 // ---------------------------------------------------------------------------------------------
 template <typename real, int QT, bool WALLS, int MODE>
 __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const StepArgs<real> A) {
-    const int gtid = blockIdx.x * kBlock + threadIdx.x;
-    if (gtid >= A.ncell) return;
+    const int gtid = A.cell0 + blockIdx.x * kBlock + threadIdx.x;
+    if (gtid >= A.cell1) return;
     const long long N = A.ncell;
     Nbh<WALLS> nb;
     nb.init(A, gtid);
@@ -339,11 +339,11 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
     extern __shared__ __align__(16) unsigned char smem_raw_async[];
     real* stage = reinterpret_cast<real*>(smem_raw_async);     // [54 + QT][kBlock]
     const int tid = threadIdx.x;
-    const int gtid = blockIdx.x * kBlock + tid;
-    const bool active = gtid < A.ncell;
+    const int gtid = A.cell0 + blockIdx.x * kBlock + tid;
+    const bool active = gtid < A.cell1;
     const long long N = A.ncell;
     Nbh<WALLS> nb;
-    nb.init(A, active ? gtid : A.ncell - 1);                   // tail lanes shadow the last cell, store nothing
+    nb.init(A, active ? gtid : A.cell1 - 1);                   // tail lanes shadow the last cell, store nothing
     const int cell = nb.idx;
 
     // Where the pre-collision population of direction q lives (AA in-place streaming, is a

@@ -107,24 +107,34 @@ int tcp_relax_temperature(tcp_sim *s, int nsteps);
  * takes the place of the periodic wrap / wall of bc[2] on that face (a face without ghost plane keeps bc[2]).
  * Arrays passed to tcp_init_fields / tcp_set_heat_source / returned by tcp_read_fields include the ghost
  * planes (initial phi, T there = the neighbour's values; p is undefined there); wall-temperature planes of the
- * x and y walls include the ghost rows.  Two-grid streaming and a thermal LB only (TCP_EUNSUPPORTED otherwise).
+ * x and y walls include the ghost rows.  Two-grid streaming only (TCP_EUNSUPPORTED with TCP_STREAM_AA).
  *
- * One message per face and step: [9 h~ planes][9 g~ planes][1, 5, 5 or 9 f~ planes][phi][T], nx*ny values each,
- * = tcp_halo_bytes.  `send_*` / `recv_*` are caller-owned DEVICE buffers of that size (NULL for a face without
- * ghost plane); `comm_stream` is the caller's cudaStream_t on which the library packs and unpacks and on which
- * the caller must enqueue the transfer send_hi -> upper neighbour's recv_lo, send_lo -> lower neighbour's
- * recv_hi between tcp_step_begin and tcp_step_end.  lo = hi = 0 turns the slab back into a plain box. */
+ * A step has `tcp_halo_phases` phases, each followed by one message per face: 1 on the thermal LB paths (the
+ * fused kernel; message [9 h~ planes][9 g~ planes][1, 5, 5 or 9 f~ planes][phi][T], nx*ny values each), 3 / 5 on
+ * the RK2 / RK4 paths (Algorithm 2: the fused phase + hydro kernel with message [9 h~][9 g~][phi], then every
+ * Runge-Kutta stage with its output plane as message, because the next stage differentiates it).
+ * `tcp_halo_message_bytes` gives the size of a phase's message, `tcp_halo_bytes` that of the largest (phase 0).
+ * `send_*` / `recv_*` are caller-owned DEVICE buffers of tcp_halo_bytes (NULL for a face without ghost plane);
+ * `comm_stream` is the caller's cudaStream_t on which the library gathers and scatters and on which the caller
+ * must enqueue, after every phase, the transfer of the first tcp_halo_message_bytes of send_hi -> the upper
+ * neighbour's recv_lo and of send_lo -> the lower neighbour's recv_hi.  lo = hi = 0 makes it a plain box again. */
 int tcp_set_halo(tcp_sim *s, int lo, int hi, void *comm_stream, void *send_lo, void *send_hi, void *recv_lo,
                  void *recv_hi);
+int tcp_halo_phases(const tcp_sim *s, int *phases);
+int tcp_halo_message_bytes(const tcp_sim *s, int phase, size_t *bytes);
 int tcp_halo_bytes(const tcp_sim *s, size_t *bytes);
 
-/* One time step of a slab, in two calls.  tcp_step_begin: the fused step on the plane(s) next to a ghost plane
- * (simulation's stream), then -- on comm_stream, as soon as those are done -- the gather of the new boundary
- * populations into send_lo / send_hi, and on the simulation's stream the fused step on the interior planes.
- * tcp_step_end: scatter recv_lo / recv_hi into the ghost planes of the new time level (comm_stream, i.e. after
- * the transfer the caller enqueued there); the simulation's stream then waits for it.  Both asynchronous.
- * tcp_step returns TCP_ESTATE on a slab; these return TCP_ESTATE on a plain box or when called out of order. */
+/* One time step of a slab: tcp_step_begin, then, after each transfer, tcp_step_advance until it reports 0
+ * transfers left.  tcp_step_begin runs phase 0: its kernel on the plane(s) next to a ghost plane (simulation's
+ * stream), then -- on comm_stream, as soon as those are done -- the gather of their new values into send_lo /
+ * send_hi, and on the simulation's stream the same kernel on the interior planes.  tcp_step_advance scatters
+ * recv_lo / recv_hi into the ghost planes (comm_stream, i.e. after the transfer the caller enqueued there; the
+ * simulation's stream then waits for it) and either runs the next phase the same way (*transfers_left >= 1) or
+ * completes the step (*transfers_left = 0).  tcp_step_end = the tcp_step_advance that completes the step
+ * (TCP_ESTATE if phases remain; all a thermal LB slab needs).  All asynchronous.  tcp_step returns TCP_ESTATE
+ * on a slab; these return TCP_ESTATE on a plain box or when called out of order. */
 int tcp_step_begin(tcp_sim *s);
+int tcp_step_advance(tcp_sim *s, int *transfers_left);
 int tcp_step_end(tcp_sim *s);
 
 /* Copy out phi, u, p = c_s^2 rho(phi) sum_i g~_i, T; any pointer may be NULL.

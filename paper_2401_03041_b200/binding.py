@@ -81,7 +81,8 @@ def make_params(d: dict) -> tcp_params:
 EXPORTS = ["tcp_workspace_bytes", "tcp_create", "tcp_create_in", "tcp_init_fields", "tcp_set_wall_temperature",
            "tcp_set_heat_source", "tcp_step", "tcp_relax_temperature", "tcp_read_fields", "tcp_synchronize", "tcp_launch_count",
            "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_destroy", "tcp_last_error",
-           "tcp_set_halo", "tcp_halo_bytes", "tcp_step_begin", "tcp_step_end"]
+           "tcp_set_halo", "tcp_halo_phases", "tcp_halo_message_bytes", "tcp_halo_bytes", "tcp_step_begin", "tcp_step_advance",
+           "tcp_step_end"]
 
 _lib = None
 
@@ -114,6 +115,9 @@ def lib():
         L.tcp_destroy.argtypes = [vp]
         L.tcp_set_halo.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp]
         L.tcp_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+        L.tcp_halo_phases.argtypes = [vp, C.POINTER(C.c_int)]
+        L.tcp_halo_message_bytes.argtypes = [vp, C.c_int, C.POINTER(C.c_size_t)]
+        L.tcp_step_advance.argtypes = [vp, C.POINTER(C.c_int)]
         L.tcp_step_begin.argtypes = [vp]
         L.tcp_step_end.argtypes = [vp]
         L.tcp_last_error.restype = C.c_char_p
@@ -220,8 +224,27 @@ def tcp_halo_bytes(sim) -> int:
     return n.value
 
 
+def tcp_halo_phases(sim) -> int:
+    n = C.c_int()
+    _check(lib().tcp_halo_phases(sim, C.byref(n)))
+    return n.value
+
+
+def tcp_halo_message_bytes(sim, phase) -> int:
+    n = C.c_size_t()
+    _check(lib().tcp_halo_message_bytes(sim, int(phase), C.byref(n)))
+    return n.value
+
+
 def tcp_step_begin(sim):
     _check(lib().tcp_step_begin(sim))
+
+
+def tcp_step_advance(sim) -> int:
+    """-> transfers left in this step (0: the step is complete)"""
+    n = C.c_int()
+    _check(lib().tcp_step_advance(sim, C.byref(n)))
+    return n.value
 
 
 def tcp_step_end(sim):

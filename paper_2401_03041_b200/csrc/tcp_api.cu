@@ -117,7 +117,8 @@ struct tcp_sim {
     int aa_next;             // AA streaming: type of the next step (1 even, 2 odd); 0 = two-grid
     // z-slab of a decomposed box (tcp_set_halo): plane 0 / nz-1 is a ghost plane filled from a neighbour
     bool halo[2];
-    bool in_step;            // between tcp_step_begin and tcp_step_end
+    bool in_step;            // between tcp_step_begin and the tcp_step_advance / tcp_step_end that completes the step
+    int phase;               // whose message is in flight (0 fused kernel, k = Runge-Kutta stage k)
     cudaStream_t comm;       // caller's stream for pack / exchange / unpack
     void* send[2];           // caller's device buffers, one message each
     void* recv[2];
@@ -174,53 +175,60 @@ unsigned grid_for(size_t n) { return (unsigned)((n + tcp::kBlock - 1) / tcp::kBl
 
 template <typename real>
 void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
+    const int P = s->nx * s->ny, planes = (R.S.cell1 - R.S.cell0) / P;       // whole planes [cell0, cell1)
     if (s->use_async) {   // default: z-marching tile kernel (tcp_rk.cuh)
         const dim3 block(tcp::kRkTX, tcp::kRkTY);
-        const dim3 grid((s->nx + tcp::kRkTX - 1) / tcp::kRkTX, (s->ny + tcp::kRkTY - 1) / tcp::kRkTY, (s->nz + tcp::kRkCZ - 1) / tcp::kRkCZ);
+        const dim3 grid((s->nx + tcp::kRkTX - 1) / tcp::kRkTX, (s->ny + tcp::kRkTY - 1) / tcp::kRkTY, (planes + tcp::kRkCZ - 1) / tcp::kRkCZ);
         if (s->walls) tcp::rk_stage_march_kernel<real, true><<<grid, block, 0, s->stream>>>(R);
         else tcp::rk_stage_march_kernel<real, false><<<grid, block, 0, s->stream>>>(R);
         return;
     }
-    const unsigned grid = grid_for(s->N);
+    const unsigned grid = grid_for((size_t)(R.S.cell1 - R.S.cell0));
     if (s->walls) tcp::rk_stage_kernel<real, true><<<grid, tcp::kBlock, 0, s->stream>>>(R);
     else tcp::rk_stage_kernel<real, false><<<grid, tcp::kBlock, 0, s->stream>>>(R);
 }
 
+// The stages of the Runge-Kutta update of T (eqs. 25-26) from T[curT] into T[1 - curT], in order;
+// phi = the phi to differentiate.  Returns their number (0 on the thermal LB paths).
+template <typename real>
+int rk_stages(const tcp_sim* s, const tcp::StepArgs<real>& A, const real* phi, tcp::RkArgs<real> st[4]) {
+    const int th = s->P.thermal;
+    if (th != TCP_THERMAL_RK2 && th != TCP_THERMAL_RK4) return 0;
+    tcp::RkArgs<real> R;
+    std::memset(&R, 0, sizeof R);
+    R.S = A;
+    R.S.phi_in = phi;
+    real* Tn = ptr<real>(s, s->L.T[s->curT]);
+    real* Tnew = ptr<real>(s, s->L.T[1 - s->curT]);
+    real* Ya = ptr<real>(s, s->L.rk[0]);
+    R.Tn = Tn;
+    if (th == TCP_THERMAL_RK2) {         // eq. 26 (G6)
+        R.Y = Tn; R.out = Ya; R.c_out = (real)0.5; R.mode = 0;
+        st[0] = R;
+        R.Y = Ya; R.out = Tnew; R.c_out = (real)1.0; R.mode = 0;
+        st[1] = R;
+        return 2;
+    }
+    real* Yb = ptr<real>(s, s->L.rk[1]);   // eq. 25
+    real* acc = ptr<real>(s, s->L.rk[2]);
+    R.acc_in = acc; R.acc_out = acc;
+    R.Y = Tn; R.out = Ya; R.c_out = (real)0.5; R.c_acc = (real)(1.0 / 6.0); R.mode = 1;
+    st[0] = R;
+    R.Y = Ya; R.out = Yb; R.c_out = (real)0.5; R.c_acc = (real)(1.0 / 3.0); R.mode = 2;
+    st[1] = R;
+    R.Y = Yb; R.out = Ya; R.c_out = (real)1.0; R.c_acc = (real)(1.0 / 3.0); R.mode = 2;
+    st[2] = R;
+    R.Y = Ya; R.out = Tnew; R.c_acc = (real)(1.0 / 6.0); R.mode = 3;
+    st[3] = R;
+    return 4;
+}
 
-// Runge-Kutta update of T (eqs. 25-26) from T[curT] into T[1 - curT]; phi = the phi to differentiate
 template <typename real>
 void rk_update(tcp_sim* s, const tcp::StepArgs<real>& A, const real* phi) {
-    const int th = s->P.thermal;
-    if (th == TCP_THERMAL_RK2 || th == TCP_THERMAL_RK4) {
-        tcp::RkArgs<real> R;
-        std::memset(&R, 0, sizeof R);
-        R.S = A;
-        R.S.phi_in = phi;
-        real* Tn = ptr<real>(s, s->L.T[s->curT]);
-        real* Tnew = ptr<real>(s, s->L.T[1 - s->curT]);
-        real* Ya = ptr<real>(s, s->L.rk[0]);
-        R.Tn = Tn;
-        if (th == TCP_THERMAL_RK2) {         // eq. 26 (G6)
-            R.Y = Tn; R.out = Ya; R.c_out = (real)0.5; R.mode = 0;
-            launch_rk_stage<real>(s, R);
-            R.Y = Ya; R.out = Tnew; R.c_out = (real)1.0; R.mode = 0;
-            launch_rk_stage<real>(s, R);
-            s->launches += 2;
-        } else {                             // eq. 25
-            real* Yb = ptr<real>(s, s->L.rk[1]);
-            real* acc = ptr<real>(s, s->L.rk[2]);
-            R.acc_in = acc; R.acc_out = acc;
-            R.Y = Tn; R.out = Ya; R.c_out = (real)0.5; R.c_acc = (real)(1.0 / 6.0); R.mode = 1;
-            launch_rk_stage<real>(s, R);
-            R.Y = Ya; R.out = Yb; R.c_out = (real)0.5; R.c_acc = (real)(1.0 / 3.0); R.mode = 2;
-            launch_rk_stage<real>(s, R);
-            R.Y = Yb; R.out = Ya; R.c_out = (real)1.0; R.c_acc = (real)(1.0 / 3.0); R.mode = 2;
-            launch_rk_stage<real>(s, R);
-            R.Y = Ya; R.out = Tnew; R.c_acc = (real)(1.0 / 6.0); R.mode = 3;
-            launch_rk_stage<real>(s, R);
-            s->launches += 4;
-        }
-    }
+    tcp::RkArgs<real> st[4];
+    const int n = rk_stages<real>(s, A, phi, st);
+    for (int i = 0; i < n; ++i) launch_rk_stage<real>(s, st[i]);
+    s->launches += n;
 }
 
 // temperature update alone, phi / u / h~ / g~ frozen
@@ -281,31 +289,53 @@ int step_once(tcp_sim* s) {
     return TCP_OK;
 }
 
-// ---- z-slab with ghost planes (tcp_set_halo): Algorithm 1's order -- boundary cells first, their
-// populations on the way to the neighbour while the interior is updated -----------------
+// ---- z-slab with ghost planes (tcp_set_halo): Algorithm 1 / 2's order -- boundary cells first, their
+// values on the way to the neighbour while the interior is updated.  A step has one
+// phase on the thermal LB paths (the fused kernel) and 1 + the number of stages on the Runge-Kutta paths
+// (fused phase + hydro kernel, then every stage: its output is differentiated by the next one) ------------
 
-// message travelling in direction dir (+1 up, -1 down): [h~ c_z=dir][g~ c_z=dir][f~ c_z=dir][phi][T], one
-// z-plane each; `gather` copies plane z of the grid into the message, otherwise the message into plane z
+int halo_phases(const tcp_sim* s) {
+    return s->P.thermal == TCP_THERMAL_RK2 ? 3 : (s->P.thermal == TCP_THERMAL_RK4 ? 5 : 1);
+}
+
+// The arrays (pointers to their plane z = 0) of which one z-plane travels in direction dir (+1 up, -1 down)
+// after phase p: [h~ c_z=dir][g~ c_z=dir][f~ c_z=dir][phi][T] of the new time level, or the stage's output.
 template <typename real>
-void halo_planes(const tcp_sim* s, tcp::HaloCopy& C, int dir, int z, int grid, int gridT, void* message, bool gather) {
-    const size_t P = (size_t)s->nx * s->ny, N = s->N;
-    real* msg = static_cast<real*>(message);
+int phase_message(const tcp_sim* s, int p, int dir, real* fields[32]) {
+    const size_t N = s->N;
+    const int o = 1 - s->cur, oT = 1 - s->curT;
     int m = 0;
-    auto add = [&](real* plane) {
-        real* in_msg = msg + (size_t)m++ * P;
+    if (p > 0) {
+        tcp::RkArgs<real> st[4];
+        rk_stages<real>(s, make_args<real>(s), nullptr, st);
+        fields[m++] = st[p - 1].out;
+        return m;
+    }
+    for (int q = 0; q < 27; ++q)
+        if (tcp::cz27(q) == dir) fields[m++] = ptr<real>(s, s->L.h[o]) + q * N;
+    for (int q = 0; q < 27; ++q)
+        if (tcp::cz27(q) == dir) fields[m++] = ptr<real>(s, s->L.g[o]) + q * N;
+    const int QT = thermal_q(s->P.thermal);
+    for (int k = 0; k < QT; ++k)
+        if (tcp::cz27(tcp::q_of(QT, k)) == dir) fields[m++] = ptr<real>(s, s->L.f[oT]) + k * N;
+    fields[m++] = ptr<real>(s, s->L.phi[o]);
+    if (QT) fields[m++] = ptr<real>(s, s->L.T[oT]);
+    return m;
+}
+
+// `gather`: plane z of the travelling arrays -> message; otherwise message -> plane z
+template <typename real>
+void halo_planes(const tcp_sim* s, tcp::HaloCopy& C, int p, int dir, int z, void* message, bool gather) {
+    const size_t P = (size_t)s->nx * s->ny;
+    real* fields[32];
+    const int m = phase_message<real>(s, p, dir, fields);
+    for (int i = 0; i < m; ++i) {
+        real* plane = fields[i] + (size_t)z * P;
+        real* in_msg = static_cast<real*>(message) + (size_t)i * P;
         C.src[C.nplanes] = gather ? plane : in_msg;
         C.dst[C.nplanes] = gather ? in_msg : plane;
         C.nplanes++;
-    };
-    for (int q = 0; q < 27; ++q)
-        if (tcp::cz27(q) == dir) add(ptr<real>(s, s->L.h[grid]) + q * N + (size_t)z * P);
-    for (int q = 0; q < 27; ++q)
-        if (tcp::cz27(q) == dir) add(ptr<real>(s, s->L.g[grid]) + q * N + (size_t)z * P);
-    const int QT = thermal_q(s->P.thermal);
-    for (int k = 0; k < QT; ++k)
-        if (tcp::cz27(tcp::q_of(QT, k)) == dir) add(ptr<real>(s, s->L.f[gridT]) + k * N + (size_t)z * P);
-    add(ptr<real>(s, s->L.phi[grid]) + (size_t)z * P);
-    add(ptr<real>(s, s->L.T[gridT]) + (size_t)z * P);
+    }
 }
 
 template <typename real>
@@ -318,16 +348,21 @@ int halo_copy(tcp_sim* s, const tcp::HaloCopy& C) {
     return TCP_OK;
 }
 
+// phase p: its kernel on the boundary planes, the gather of their new values (comm stream), its kernel on the interior
 template <typename real>
-int step_begin_t(tcp_sim* s) {
+int phase_begin(tcp_sim* s, int p) {
     const int P = s->nx * s->ny;
     const int zlo = s->halo[0] ? 1 : 0, zhi = s->nz - 1 - (s->halo[1] ? 1 : 0);   // first / last plane this slab owns
     tcp::StepArgs<real> A = make_args<real>(s);
-    CK(cudaEventRecord(s->ev0, s->stream));
-    auto planes = [&](int z0, int z1) {       // update the planes z0..z1
+    auto planes = [&](int z0, int z1) {       // run the phase on the planes z0..z1
         if (z1 < z0) return (int)TCP_OK;
         A.cell0 = z0 * P; A.cell1 = (z1 + 1) * P;
-        return launch_fused<real>(s, A);
+        if (p == 0) return launch_fused<real>(s, A);
+        tcp::RkArgs<real> st[4];
+        rk_stages<real>(s, A, A.phi_out, st);
+        launch_rk_stage<real>(s, st[p - 1]);
+        s->launches++;
+        return (int)TCP_OK;
     };
     int rc = TCP_OK;
     if (s->halo[0]) rc = planes(zlo, zlo);
@@ -338,34 +373,58 @@ int step_begin_t(tcp_sim* s) {
     tcp::HaloCopy C;
     std::memset(&C, 0, sizeof C);
     C.plane_cells = P;
-    const int o = 1 - s->cur, oT = 1 - s->curT;                                    // the grids this step writes
-    if (s->halo[0]) halo_planes<real>(s, C, -1, zlo, o, oT, s->send[0], true);
-    if (s->halo[1]) halo_planes<real>(s, C, +1, zhi, o, oT, s->send[1], true);
+    if (s->halo[0]) halo_planes<real>(s, C, p, -1, zlo, s->send[0], true);
+    if (s->halo[1]) halo_planes<real>(s, C, p, +1, zhi, s->send[1], true);
     rc = halo_copy<real>(s, C);
     if (rc) return rc;
     rc = planes(zlo + (s->halo[0] ? 1 : 0), zhi - (s->halo[1] ? 1 : 0));
     if (rc) return rc;
-    s->in_step = true;
+    CK(cudaGetLastError());
     return TCP_OK;
 }
 
+// the message of phase p has been transferred (enqueued on the comm stream): scatter it into the ghost planes
 template <typename real>
-int step_end_t(tcp_sim* s) {
+int phase_end(tcp_sim* s, int p) {
     tcp::HaloCopy C;
     std::memset(&C, 0, sizeof C);
     C.plane_cells = s->nx * s->ny;
-    const int o = 1 - s->cur, oT = 1 - s->curT;
-    if (s->halo[0]) halo_planes<real>(s, C, +1, 0, o, oT, s->recv[0], false);          // from below, moving up
-    if (s->halo[1]) halo_planes<real>(s, C, -1, s->nz - 1, o, oT, s->recv[1], false);  // from above, moving down
+    if (s->halo[0]) halo_planes<real>(s, C, p, +1, 0, s->recv[0], false);          // from below, moving up
+    if (s->halo[1]) halo_planes<real>(s, C, p, -1, s->nz - 1, s->recv[1], false);  // from above, moving down
     int rc = halo_copy<real>(s, C);
     if (rc) return rc;
     CK(cudaEventRecord(s->ev_comm, s->comm));
     CK(cudaStreamWaitEvent(s->stream, s->ev_comm, 0));
+    return TCP_OK;
+}
+
+template <typename real>
+int step_begin_t(tcp_sim* s) {
+    CK(cudaEventRecord(s->ev0, s->stream));
+    int rc = phase_begin<real>(s, 0);
+    if (rc) return rc;
+    s->in_step = true;
+    s->phase = 0;
+    return TCP_OK;
+}
+
+template <typename real>
+int step_advance_t(tcp_sim* s, int* transfers_left) {
+    int rc = phase_end<real>(s, s->phase);
+    if (rc) return rc;
+    if (s->phase + 1 < halo_phases(s)) {
+        rc = phase_begin<real>(s, s->phase + 1);
+        if (rc) return rc;
+        s->phase++;
+        *transfers_left = halo_phases(s) - s->phase;
+        return TCP_OK;
+    }
     CK(cudaEventRecord(s->ev1, s->stream));
     s->cur = 1 - s->cur;
     s->curT = 1 - s->curT;
     s->in_step = false;
     s->stepped = true;
+    *transfers_left = 0;
     return TCP_OK;
 }
 
@@ -593,13 +652,22 @@ int tcp_synchronize(tcp_sim* s) {
 
 long long tcp_launch_count(const tcp_sim* s) { return s ? s->launches : 0; }
 
-int tcp_halo_bytes(const tcp_sim* s, size_t* bytes) {
+int tcp_halo_phases(const tcp_sim* s, int* phases) {
+    if (!s || !phases) return fail(TCP_EINVAL, "NULL argument");
+    *phases = halo_phases(s);
+    return TCP_OK;
+}
+
+int tcp_halo_message_bytes(const tcp_sim* s, int phase, size_t* bytes) {
     if (!s || !bytes) return fail(TCP_EINVAL, "NULL argument");
+    if (phase < 0 || phase >= halo_phases(s)) return fail(TCP_EINVAL, "phase out of range (tcp_halo_phases)");
     const int QT = thermal_q(s->P.thermal);
-    const size_t planes = 9 + 9 + (size_t)tcp::halo_crossing(QT, 1) + 2;
+    const size_t planes = phase > 0 ? 1 : 9 + 9 + (size_t)tcp::halo_crossing(QT, 1) + 1 + (QT ? 1 : 0);
     *bytes = planes * s->nx * s->ny * (s->P.precision == TCP_F64 ? 8 : 4);
     return TCP_OK;
 }
+
+int tcp_halo_bytes(const tcp_sim* s, size_t* bytes) { return tcp_halo_message_bytes(s, 0, bytes); }
 
 int tcp_set_halo(tcp_sim* s, int lo, int hi, void* comm_stream, void* send_lo, void* send_hi, void* recv_lo, void* recv_hi) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
@@ -607,7 +675,6 @@ int tcp_set_halo(tcp_sim* s, int lo, int hi, void* comm_stream, void* send_lo, v
     lo = lo != 0; hi = hi != 0;
     if (lo || hi) {
         if (s->P.streaming != TCP_STREAM_TWO_GRID) return fail(TCP_EUNSUPPORTED, "ghost planes: two-grid streaming only");
-        if (thermal_q(s->P.thermal) == 0) return fail(TCP_EUNSUPPORTED, "ghost planes: thermal LB only (the Runge-Kutta stages would need an exchange per stage)");
         if (s->nz - lo - hi < 1) return fail(TCP_EINVAL, "a slab needs at least one plane of its own between its ghost planes");
         if ((lo && (!send_lo || !recv_lo)) || (hi && (!send_hi || !recv_hi))) return fail(TCP_EINVAL, "a face with a ghost plane needs a send and a receive buffer");
     }
@@ -625,10 +692,18 @@ int tcp_step_begin(tcp_sim* s) {
     return s->P.precision == TCP_F64 ? step_begin_t<double>(s) : step_begin_t<float>(s);
 }
 
+int tcp_step_advance(tcp_sim* s, int* transfers_left) {
+    if (!s || !transfers_left) return fail(TCP_EINVAL, "NULL argument");
+    if (!s->in_step) return fail(TCP_ESTATE, "tcp_step_advance without tcp_step_begin");
+    return s->P.precision == TCP_F64 ? step_advance_t<double>(s, transfers_left) : step_advance_t<float>(s, transfers_left);
+}
+
 int tcp_step_end(tcp_sim* s) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
     if (!s->in_step) return fail(TCP_ESTATE, "tcp_step_end without tcp_step_begin");
-    return s->P.precision == TCP_F64 ? step_end_t<double>(s) : step_end_t<float>(s);
+    if (s->phase + 1 < halo_phases(s)) return fail(TCP_ESTATE, "tcp_step_end: Runge-Kutta stages (and their transfers) are still to come, use tcp_step_advance");
+    int left = 0;
+    return tcp_step_advance(s, &left);
 }
 
 int tcp_pattern_copy_ms(tcp_sim* s, int nlaunches, float* ms) {

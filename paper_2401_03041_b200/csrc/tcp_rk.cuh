@@ -31,8 +31,10 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, TCP_RK_MINB) rk_stage_march_ker
     constexpr int TX = kRkTX, TY = kRkTY, PX = TX + 2, PY = TY + 2, PE = PX * PY;
     __shared__ real tileY[2][PE], tileP[2][PE];
     const int tid = threadIdx.y * TX + threadIdx.x;
-    const int bx0 = blockIdx.x * TX, by0 = blockIdx.y * TY, z0 = blockIdx.z * kRkCZ;
-    const int nzc = min(kRkCZ, A.nz - z0);
+    // planes [cell0, cell1) / (nx ny): the whole box, or the boundary planes / the interior of a slab
+    const int zfirst = A.cell0 / (A.nx * A.ny), zend = A.cell1 / (A.nx * A.ny);
+    const int bx0 = blockIdx.x * TX, by0 = blockIdx.y * TY, z0 = zfirst + blockIdx.z * kRkCZ;
+    const int nzc = min(kRkCZ, zend - z0);
     const int x = bx0 + threadIdx.x, y = by0 + threadIdx.y;
     const bool inside = x < A.nx && y < A.ny;
     const long long N = A.ncell;

@@ -542,8 +542,8 @@ struct RkArgs {
 template <typename real, bool WALLS>
 __global__ void __launch_bounds__(kBlock) rk_stage_kernel(const RkArgs<real> R) {
     const StepArgs<real>& A = R.S;
-    const int gtid = blockIdx.x * kBlock + threadIdx.x;
-    if (gtid >= A.ncell) return;
+    const int gtid = A.cell0 + blockIdx.x * kBlock + threadIdx.x;
+    if (gtid >= A.cell1) return;
     const long long N = A.ncell;
     Nbh<WALLS> nb;
     nb.init(A, gtid);

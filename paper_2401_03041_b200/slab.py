@@ -2,7 +2,8 @@
 
 A box of nz planes is cut into `world` z-slabs.  Every slab is an ordinary `tcp_sim` with one ghost plane on
 each face that has a neighbour (`tcp_set_halo`); one step is `tcp_step_begin` (boundary planes, gather, interior)
--> the transfer of one message per face -> `tcp_step_end` (scatter).  This module only slices arrays, owns the
+-> the transfer of one message per face -> `tcp_step_advance` (scatter; on the Runge-Kutta paths then the next
+stage the same way, until no transfer is left).  This module only slices arrays, owns the
 message buffers and moves the messages: between slabs of ONE process (`LocalSlabs`, a device copy; what the
 single-GPU tests and `bench.py --slabs` run) or between ranks (`RankSlab`, `torch.distributed` point-to-point,
 NCCL over NVLink on GPUs).  No arithmetic of the method lives here.
@@ -107,6 +108,9 @@ class Slab:
         self.send_lo, self.recv_lo, self.send_hi, self.recv_hi = mk(self.lo), mk(self.lo), mk(self.hi), mk(self.hi)
         if self.lo or self.hi:
             B.tcp_set_halo(self.sim._h, self.lo, self.hi, self.comm, self.send_lo, self.send_hi, self.recv_lo, self.recv_hi)
+        # values of the message that follows each phase of a step (tcp_halo_message_bytes)
+        item = np.dtype(self.sim.np_dtype).itemsize
+        self.message_values = [B.tcp_halo_message_bytes(self.sim._h, p) // item for p in range(B.tcp_halo_phases(self.sim._h))]
 
     @property
     def halo(self):
@@ -142,9 +146,9 @@ class Slab:
         else:
             self.sim.step(1)
 
-    def step_end(self):
-        if self.halo:
-            B.tcp_step_end(self.sim._h)
+    def step_advance(self) -> int:
+        """After a transfer: scatter, then the next phase or the end of the step.  -> transfers left"""
+        return B.tcp_step_advance(self.sim._h) if self.halo else 0
 
     def read_fields(self):
         """phi, u, p, T of the planes this slab owns (host arrays)."""
@@ -180,15 +184,16 @@ class LocalSlabs:
         for _ in range(n):
             for s in self.slabs:
                 s.step_begin()
-            with torch.cuda.stream(self.comm):      # after every gather, before every scatter (same stream)
+            for nv in self.slabs[0].message_values:     # one transfer after every phase
+                with torch.cuda.stream(self.comm):      # after every gather, before every scatter (same stream)
+                    for s in self.slabs:
+                        lower, upper = self.layout.neighbours(s.rank)
+                        if s.hi:
+                            self.slabs[upper].recv_lo[:nv].copy_(s.send_hi[:nv], non_blocking=True)
+                        if s.lo:
+                            self.slabs[lower].recv_hi[:nv].copy_(s.send_lo[:nv], non_blocking=True)
                 for s in self.slabs:
-                    lower, upper = self.layout.neighbours(s.rank)
-                    if s.hi:
-                        self.slabs[upper].recv_lo.copy_(s.send_hi, non_blocking=True)
-                    if s.lo:
-                        self.slabs[lower].recv_hi.copy_(s.send_lo, non_blocking=True)
-            for s in self.slabs:
-                s.step_end()
+                    s.step_advance()
 
     def read_fields(self):
         parts = [s.read_fields() for s in self.slabs]
@@ -229,10 +234,14 @@ class RankSlab:
         s = self.slab
         for _ in range(n):
             s.step_begin()
-            if s.halo:
+            if not s.halo:
+                continue
+            cut = lambda t, nv: None if t is None else t[:nv]
+            for nv in s.message_values:
                 with torch.cuda.stream(s.comm):
-                    exchange_faces(s.send_lo, s.send_hi, s.recv_lo, s.recv_hi, self.lower, self.upper, self.group)
-            s.step_end()
+                    exchange_faces(cut(s.send_lo, nv), cut(s.send_hi, nv), cut(s.recv_lo, nv), cut(s.recv_hi, nv),
+                                   self.lower, self.upper, self.group)
+                s.step_advance()
 
     def close(self):
         self.slab.close()

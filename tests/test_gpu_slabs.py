@@ -105,6 +105,51 @@ def test_fp32_slabs(kernel, monkeypatch):
     assert_same_bits(got, want)
 
 
+@pytest.mark.parametrize("thermal", ["rk2", "rk4"])
+@pytest.mark.parametrize("kernel", ["march", "flat"])
+def test_runge_kutta_slabs(thermal, kernel, monkeypatch):
+    # Algorithm 2: one transfer after the fused kernel and one after every stage (3 / 5 per step)
+    if kernel == "flat":
+        monkeypatch.setenv("TCP_KERNEL", "flat")
+    wl = configs.perf_box(36, thermal=thermal, ny=20, nz=23, seed=4, r_min=4.0, r_max=5.0)   # x spans two 32-wide tiles
+    want, _ = run_gpu(wl, 12)
+    got, _ = run_slabs(wl, 3, 12)
+    assert_same_bits(got, want)
+
+
+def test_runge_kutta_tweezer_walls_in_z():
+    # config-4 set-up at reduced size (RK2, wall-temperature plane on the bottom wall, initial velocity)
+    wl = configs.thermal_tweezer(nx=24, ny=20, nz=18, thermal="rk2", R=5.0, offset=4.0, A=2.0, s=5.0)
+    q = configs.laser_source(24, 20, 18, Q_s=0.01, w_s=4.0, d_s=5.0)
+    want, _ = run_gpu(wl, 20, q=q)
+    got, _ = run_slabs(wl, 4, 20, q=q)
+    assert_same_bits(got, want)
+    assert_parity_f64(got, run_oracle(wl, 20, q=q))
+
+
+def test_runge_kutta_phases_and_messages():
+    wl = configs.perf_box(16, thermal="rk4", ny=12, nz=12, seed=1, r_min=3.0, r_max=4.0)
+    box = LocalSlabs(16, 12, 12, 2, dict(wl.params))
+    h = box.slabs[0].sim._h
+    assert B.tcp_halo_phases(h) == 5
+    plane = 16 * 12 * 8
+    assert [B.tcp_halo_message_bytes(h, p) for p in range(5)] == [19 * plane] + [plane] * 4
+    assert B.tcp_halo_bytes(h) == 19 * plane
+    box.init_fields(_np(wl.phi), None, _np(wl.T))
+    B.tcp_step_begin(h)
+    with pytest.raises(tcp.TcpError) as e:
+        B.tcp_step_end(h)                      # four stages and their transfers are still to come
+    assert e.value.code == B.TCP_ESTATE
+    assert [B.tcp_step_advance(h) for _ in range(5)] == [4, 3, 2, 1, 0]
+    with pytest.raises(tcp.TcpError) as e:
+        B.tcp_step_advance(h)
+    assert e.value.code == B.TCP_ESTATE
+    box.close()
+    box = LocalSlabs(16, 12, 12, 2, dict(wl.params, thermal="rk2"))
+    assert B.tcp_halo_phases(box.slabs[0].sim._h) == 3
+    box.close()
+
+
 def test_general_rates_and_bgk_in_slabs():
     wl = configs.perf_box(16, thermal="lb_d3q7", ny=14, nz=12, seed=9, r_min=3.0, r_max=4.0)
     for extra in (dict(s_high=1.5, s_bulk=0.8), dict(high_rate_equals_shear=1)):
@@ -152,19 +197,18 @@ def test_state_errors():
         B.tcp_relax_temperature(h, 2)
     assert e.value.code == B.TCP_EUNSUPPORTED
     box.close()
-    # a plain box has no split step; Runge-Kutta and AA boxes take no ghost planes
+    # a plain box has no split step; AA boxes take no ghost planes
     sim = tcp.Simulation(16, 12, 8, dict(wl.params))
     with pytest.raises(tcp.TcpError) as e:
         B.tcp_step_begin(sim._h)
     assert e.value.code == B.TCP_ESTATE
     sim.close()
     buf = torch.zeros(64 * 16 * 12, dtype=torch.float64, device="cuda")
-    for extra in (dict(thermal="rk2"), dict(streaming="aa")):
-        sim = tcp.Simulation(16, 12, 8, dict(wl.params, **extra))
-        with pytest.raises(tcp.TcpError) as e:
-            B.tcp_set_halo(sim._h, 1, 1, torch.cuda.Stream(), buf, buf, buf, buf)
-        assert e.value.code == B.TCP_EUNSUPPORTED
-        sim.close()
+    sim = tcp.Simulation(16, 12, 8, dict(wl.params, streaming="aa"))
+    with pytest.raises(tcp.TcpError) as e:
+        B.tcp_set_halo(sim._h, 1, 1, torch.cuda.Stream(), buf, buf, buf, buf)
+    assert e.value.code == B.TCP_EUNSUPPORTED
+    sim.close()
     sim = tcp.Simulation(16, 12, 2, dict(wl.params))
     with pytest.raises(tcp.TcpError) as e:
         B.tcp_set_halo(sim._h, 1, 1, torch.cuda.Stream(), buf, buf, buf, buf)     # no plane of its own left

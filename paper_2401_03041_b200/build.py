@@ -16,7 +16,7 @@ LIB = os.path.join(HERE, "libtcp.so")
 SOURCES = ["tcp_api.cu", "tcp_fused_f64_periodic.cu", "tcp_fused_f64_walls.cu", "tcp_fused_f32_periodic.cu",
            "tcp_fused_f32_walls.cu"]
 HEADERS = ["tcp_lattice.cuh", "tcp_device.cuh", "tcp_kernels.cuh", "tcp_step.cuh", "tcp_rk.cuh",
-           "tcp_launch.h", "tcp_launch.inl", "tcp_real.cuh", "tcp_pair.cuh"]
+           "tcp_launch.h", "tcp_launch.inl", "tcp_real.cuh", "tcp_pair.cuh", "tcp_halo.cuh"]
 # IEEE division / sqrt kept (no fast-math); FMA contraction on
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo", "-fmad=true",
               "-Xcompiler", "-fPIC"]

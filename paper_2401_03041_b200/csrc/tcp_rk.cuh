@@ -13,12 +13,12 @@
 
 namespace tcp {
 
-constexpr int kRkTX = 32, kRkTY = 8, kRkCZ = 32;
-// 92 registers without a bound = 2 blocks of 256 per SM and 61 % of cycles without an eligible warp (ncu);
-// 3 blocks cost 48 B of spills
-#ifndef TCP_RK_MINB
-#define TCP_RK_MINB 3
-#endif
+constexpr int kRkTX = 32, kRkTY = 8, kRkCZ = 32;   // chunks of 16-100 planes: within 1 % (profiles/r01_notes.md section 8)
+// Residency (profiles/r01_notes.md section 8): with the cell data requested one plane ahead the fp64 kernel needs
+// 119 registers -> 2 blocks of 256 per SM without spills (3 blocks: 80-116 B of spills and 8-15 % slower);
+// the fp32 kernel fits 3 blocks.
+template <typename real>
+constexpr int rk_min_blocks() { return sizeof(real) == 8 ? 2 : 3; }
 
 template <typename real>
 struct Plane3 {          // in-plane reductions of one field on one z plane
@@ -26,7 +26,7 @@ struct Plane3 {          // in-plane reductions of one field on one z plane
 };
 
 template <typename real, bool WALLS>
-__global__ void __launch_bounds__(kRkTX * kRkTY, TCP_RK_MINB) rk_stage_march_kernel(const RkArgs<real> R) {
+__global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage_march_kernel(const RkArgs<real> R) {
     const StepArgs<real>& A = R.S;
     constexpr int TX = kRkTX, TY = kRkTY, PX = TX + 2, PY = TY + 2, PE = PX * PY;
     __shared__ real tileY[2][PE], tileP[2][PE];
@@ -111,17 +111,22 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, TCP_RK_MINB) rk_stage_march_ker
     Ym = reduce_plane(tileY[0]); Pm = reduce_plane(tileP[0]);
     Yc = reduce_plane(tileY[1]); Pc = reduce_plane(tileP[1]);
     __syncthreads();                       // buffer 0 may now be overwritten
+    // cell data (u, T^n, accumulator, source) of plane z0 + k are requested one iteration ahead as well
+    real nu[3] = {real(0), real(0), real(0)}, nTn = real(0), nacc = real(0), nq = real(0);
+    auto fetch_cell = [&](int zz) {
+        if (!inside) return;
+        const int c = x + sy * y + sz * zz;
+        nu[0] = A.u[c]; nu[1] = A.u[N + c]; nu[2] = A.u[2 * N + c];
+        nTn = R.Tn[c];
+        if (R.mode >= 2) nacc = R.acc_in[c];
+        if (A.q_src) nq = A.q_src[c];
+    };
+    fetch_cell(z0);
     for (int k = 0; k < nzc; ++k) {
         const int buf = k & 1;
-        // cell data of plane z0 + k, requested before the barrier so that its latency hides behind it
         const int cell = x + sy * y + sz * (z0 + k);
-        real u[3] = {real(0), real(0), real(0)}, Tn = real(0), acc = real(0), qT = real(0);
-        if (inside) {
-            u[0] = A.u[cell]; u[1] = A.u[N + cell]; u[2] = A.u[2 * N + cell];
-            Tn = R.Tn[cell];
-            if (R.mode >= 2) acc = R.acc_in[cell];
-            if (A.q_src) qT = A.q_src[cell];
-        }
+        const real u[3] = {nu[0], nu[1], nu[2]}, Tn = nTn, acc = nacc, qT = nq;
+        if (k + 1 < nzc) fetch_cell(z0 + k + 1);
         store_plane(buf);                          // plane z0 + k + 1
         if (k + 1 < nzc) fetch_plane(z0 + k + 2);  // next one: its latency hides behind this iteration
         __syncthreads();

@@ -107,7 +107,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_throughput(thermal, n=40, warm=1, steps=6):
+def oracle_throughput(thermal, n=64, warm=1, steps=10):
     """The oracle, as it stands, on a bounded sample of the workload (n^3 box, same recipe)."""
     from oracle import tcpo
     wl = W.perf_box(n, thermal=thermal, r_min=4.0, r_max=8.0)
@@ -377,7 +377,7 @@ def main():
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--streaming", default="two_grid", choices=["two_grid", "aa"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-size", type=int, default=40)
+    ap.add_argument("--ref-size", type=int, default=64)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="per-variant / per-size table (configs[4]); one JSON line each")

@@ -57,6 +57,8 @@ typedef struct tcpo_params {
     int high_rate_equals_shear;        /* 1 => every rate = the physical one => BGK */
     double eps_normal;                 /* reading S8 */
     double wall_u[3][2][3];            /* wall velocity per axis / face (moving wall; reading S18) */
+    double sigma_TT;                   /* d^2 sigma / dT^2: "parabolic (or non-linear) relation between surface tension and
+                                          temperature" (reading S19); 0 = the linear eq. 9 */
 } tcpo_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -302,6 +304,16 @@ int tcpo_num_threads(void) {
     return omp_get_max_threads();
 #else
     return 1;
+#endif
+}
+
+/* Threads for the cell loops of the calls that follow (the harness uses one thread on grids too small to
+ * pay for a parallel region; the arithmetic per cell does not depend on it). */
+void tcpo_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
 #endif
 }
 
@@ -572,7 +584,11 @@ static int update_g(tcpo_sim *s) {
                 double G[3], lap, Th[3], lapT;
                 fd_ops(s, s->phi, 0, x, y, z, G, &lap);
                 fd_ops(s, s->T, 1, x, y, z, Th, &lapT);
-                double sigma = P->sigma_ref + P->sigma_T * (Tc - P->T_ref); /* eq. 9 */
+                /* eq. 9, plus the parabolic term of reading S19 (sigma_TT = 0: eq. 9 as printed);
+                 * dsigma = d sigma / dT is what multiplies the tangential (Marangoni) term of eq. 8 */
+                double dTr = Tc - P->T_ref;
+                double sigma = P->sigma_ref + P->sigma_T * dTr + 0.5 * P->sigma_TT * dTr * dTr;
+                double dsigma = P->sigma_T + P->sigma_TT * dTr;
                 double beta = 12.0 * sigma / P->xi, kphi = 1.5 * sigma * P->xi; /* S5 */
                 double mu = 4.0 * beta * ph * (ph - 1.0) * (ph - 0.5) - kphi * lap;
                 /* O6: forces.  eq. 8 (with |grad phi|^2, G2), eq. 7, eq. 20 */
@@ -580,7 +596,7 @@ static int update_g(tcpo_sim *s) {
                 double TG = Th[0] * G[0] + Th[1] * G[1] + Th[2] * G[2];
                 double F0[3], ustar[3], Fmu[3], F[3], u[3], a[3];
                 for (int al = 0; al < 3; al++) {
-                    double Fs = mu * G[al] + 1.5 * P->xi * P->sigma_T * (GG * Th[al] - TG * G[al]);
+                    double Fs = mu * G[al] + 1.5 * P->xi * dsigma * (GG * Th[al] - TG * G[al]);
                     double Fb = rho * P->gravity[al];
                     double Fp = -pstar * CS2 * drho * G[al];
                     F0[al] = Fs + Fb + Fp;

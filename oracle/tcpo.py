@@ -31,6 +31,7 @@ class Params(C.Structure):
         ("high_rate_equals_shear", C.c_int),
         ("eps_normal", C.c_double),
         ("wall_u", ((C.c_double * 3) * 2) * 3),
+        ("sigma_TT", C.c_double),
     ]
 
 
@@ -42,6 +43,7 @@ DEFAULTS = dict(
     gravity=(0.0, 0.0, 0.0), wall_T=((0.0, 0.0), (0.0, 0.0), (0.0, 0.0)),
     s_bulk=1.0, s_high=1.0, high_rate_equals_shear=0, eps_normal=1e-32,
     wall_u=(((0.0,) * 3,) * 2,) * 3,
+    sigma_TT=0.0,
 )
 
 
@@ -63,7 +65,7 @@ def make_params(d: dict) -> Params:
         p.gravity[a] = float(v["gravity"][a])
         for f in range(2):
             p.wall_T[a][f] = float(v["wall_T"][a][f])
-    for k in ("rho_H", "rho_L", "tau_H", "tau_L", "xi", "M", "sigma_ref", "sigma_T", "T_ref",
+    for k in ("rho_H", "rho_L", "tau_H", "tau_L", "xi", "M", "sigma_ref", "sigma_T", "sigma_TT", "T_ref",
               "kappa_H", "kappa_L", "cp_H", "cp_L", "s_bulk", "s_high", "eps_normal"):
         setattr(p, k, float(v[k]))
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
@@ -99,6 +101,8 @@ def lib():
         L.tcpo_fd.argtypes = [C.c_void_p, dp, C.c_int, dp, dp]
         L.tcpo_last_error.restype = C.c_char_p
         L.tcpo_num_threads.restype = C.c_int
+        L.tcpo_set_num_threads.argtypes = [C.c_int]
+        L.tcpo_set_num_threads.restype = None
         _lib = L
     return _lib
 
@@ -122,6 +126,18 @@ def _check(rc):
 
 def num_threads() -> int:
     return int(lib().tcpo_num_threads())
+
+
+_MAX_THREADS = None
+
+
+def threads_for(cells: int) -> int:
+    """One thread per 4096 cells, at most what OpenMP offers: a parallel region costs more than it saves on
+    the small grids of the pins (measured: 512 cells, 8 threads on a busy box = 6x slower than 1 thread)."""
+    global _MAX_THREADS
+    if _MAX_THREADS is None:
+        _MAX_THREADS = num_threads()
+    return max(1, min(_MAX_THREADS, cells // 4096))
 
 
 class Oracle:
@@ -162,9 +178,11 @@ class Oracle:
         _check(lib().tcpo_set_heat_source(self._h, _dp(q)))
 
     def step(self, n=1):
+        lib().tcpo_set_num_threads(threads_for(self.n))
         _check(lib().tcpo_step(self._h, int(n)))
 
     def relax_temperature(self, n=1):
+        lib().tcpo_set_num_threads(threads_for(self.n))
         _check(lib().tcpo_relax_temperature(self._h, int(n)))
 
     def read_fields(self):

@@ -60,6 +60,10 @@ typedef struct tcp_params {
     double eps_normal;                 /* n = grad phi / sqrt(|grad phi|^2 + eps); default 1e-32 */
     double wall_u[3][2][3];            /* velocity of each wall [axis][face][component] (moving wall):
                                           enters the bounce-back of g only; default 0 */
+    double sigma_TT;                   /* d^2 sigma / dT^2 of a parabolic sigma(T) = sigma_ref + sigma_T (T - T_ref)
+                                          + sigma_TT (T - T_ref)^2 / 2 (self-rewetting fluids); the
+                                          Marangoni term of eq. 8 then carries d sigma/dT = sigma_T + sigma_TT (T - T_ref).
+                                          Default 0 = eq. 9 as printed */
 } tcp_params;
 
 /* Bytes of device memory one simulation needs (populations, fields, wall planes).

@@ -151,7 +151,7 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     A.rho_L = (real)P.rho_L; A.drho = (real)(P.rho_H - P.rho_L);
     A.tau_L = (real)P.tau_L; A.dtau = (real)(P.tau_H - P.tau_L);
     A.xi = (real)P.xi; A.w_phi = (real)(1.0 / (0.5 + 3.0 * P.M));
-    A.sigma_ref = (real)P.sigma_ref; A.sigma_T = (real)P.sigma_T; A.T_ref = (real)P.T_ref;
+    A.sigma_ref = (real)P.sigma_ref; A.sigma_T = (real)P.sigma_T; A.T_ref = (real)P.T_ref; A.sigma_TT = (real)P.sigma_TT;
     A.kappa_L = (real)P.kappa_L; A.dkappa = (real)(P.kappa_H - P.kappa_L);
     A.cp_L = (real)P.cp_L; A.dcp = (real)(P.cp_H - P.cp_L);
     for (int a = 0; a < 3; ++a) A.grav[a] = (real)P.gravity[a];

@@ -29,6 +29,7 @@ struct StepArgs {
     real rho_L, drho, tau_L, dtau;   // eqs. 14, 22
     real xi, w_phi;                  // eq. 15; rate 1/(1/2 + 3M) (eq. 11, reading G3)
     real sigma_ref, sigma_T, T_ref;  // eq. 9
+    real sigma_TT;                   // parabolic sigma(T) (reading S19); 0 = eq. 9
     real kappa_L, dkappa, cp_L, dcp; // eqs. 23-24 (reading G5)
     real grav[3];                    // eq. 7
     real s_bulk, s_high, eps;
@@ -55,6 +56,7 @@ struct StepArgs<f32x2> {
     f32x2 rho_L, drho, tau_L, dtau;
     f32x2 xi, w_phi;
     f32x2 sigma_ref, sigma_T, T_ref;
+    f32x2 sigma_TT;
     f32x2 kappa_L, dkappa, cp_L, dcp;
     f32x2 grav[3];
     f32x2 s_bulk, s_high, eps;
@@ -64,7 +66,7 @@ struct StepArgs<f32x2> {
         : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), cell0(A.cell0), cell1(A.cell1), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
           f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src),
           rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), sigma_ref(A.sigma_ref),
-          sigma_T(A.sigma_T), T_ref(A.T_ref), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
+          sigma_T(A.sigma_T), T_ref(A.T_ref), sigma_TT(A.sigma_TT), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
           s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving) {
         for (int a = 0; a < 3; ++a) {
             wall[a] = A.wall[a];

@@ -125,12 +125,15 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
     const real j[3] = {M.mx, M.my, M.mz};
     const real rho = A.rho_L + phi_c * A.drho;              // eq. 14
     const real tau = A.tau_L + phi_c * A.dtau;              // eq. 22
-    const real sigma = A.sigma_ref + A.sigma_T * (T_c - A.T_ref);   // eq. 9
+    // eq. 9 plus the parabolic term of reading S19; dsigma = d sigma / dT carries the Marangoni term of eq. 8
+    const real dTr = T_c - A.T_ref;
+    const real dsigma = A.sigma_T + A.sigma_TT * dTr;
+    const real sigma = A.sigma_ref + A.sigma_T * dTr + real(0.5) * A.sigma_TT * dTr * dTr;
     // mu_phi = 4 beta phi (phi-1)(phi-1/2) - k lap phi, beta = 12 sigma/xi, k = 3 sigma xi/2  (S5)
     const real mu = real(48) * sigma / A.xi * phi_c * (phi_c - real(1)) * (phi_c - real(0.5)) - real(1.5) * sigma * A.xi * lapPhi;
     const real GG = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
     const real TG = Th[0] * G[0] + Th[1] * G[1] + Th[2] * G[2];
-    const real mar = real(1.5) * A.xi * A.sigma_T;          // eq. 8 (with |grad phi|^2, G2)
+    const real mar = real(1.5) * A.xi * dsigma;             // eq. 8 (with |grad phi|^2, G2)
     const real pcoef = ps * real(1.0 / 3.0) * A.drho;       // eq. 20
     const real i2r = real(0.5) / rho;
     real F[3], us[3];

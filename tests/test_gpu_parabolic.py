@@ -1,0 +1,42 @@
+"""Parabolic surface tension sigma_TT (reading S19) on the GPU against the oracle:
+fp64 1e-10 after 100 steps, fp32 1e-5 relative, every kernel family that carries the hydrodynamic collision."""
+import numpy as np
+import pytest
+
+import workloads as W
+from parity_util import assert_parity_f32, assert_parity_f64, run_gpu, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+# vertex inside the temperature range of the boxes below (T in [0.43, 0.58]): d sigma/dT takes both signs
+PARABOLA = dict(sigma_ref=5e-3, sigma_T=-2e-4, sigma_TT=2e-2, T_ref=0.5, eps_normal=1e-6)
+
+
+@pytest.mark.parametrize("streaming", ["two_grid", "aa"])
+@pytest.mark.parametrize("thermal", ["lb_d3q7", "lb_d3q27", "rk4"])
+def test_perf_box_with_parabolic_surface_tension(thermal, streaming):
+    wl = W.perf_box(20, thermal=thermal, ny=16, nz=14, r_min=3.0, r_max=4.0, seed=8)
+    extra = dict(PARABOLA, streaming=streaming)
+    want = run_oracle(wl, 100, extra=extra)
+    got, _ = run_gpu(wl, 100, extra=extra)
+    assert_parity_f64(got, want)
+    lin = run_oracle(wl, 100, extra=dict(extra, sigma_TT=0.0))
+    assert np.abs(want[1] - lin[1]).max() > 1e-7      # the parabolic term is felt, 1000 x above the parity bar
+
+
+def test_droplet_between_walls_general_rates_and_bgk():
+    wl = W.droplet_in_gradient(nx=18, ny=16, nz=24, thermal="lb_d3q19", R=5.0, zc=10.0, grad_T=0.05)
+    for extra in (dict(PARABOLA, s_high=1.5, s_bulk=0.8), dict(PARABOLA, high_rate_equals_shear=1)):
+        want = run_oracle(wl, 60, extra=extra)
+        got, _ = run_gpu(wl, 60, extra=extra)
+        assert_parity_f64(got, want)
+
+
+@pytest.mark.parametrize("kernel", ["pair", "scalar"])
+def test_fp32_with_parabolic_surface_tension(kernel, monkeypatch):
+    if kernel == "scalar":
+        monkeypatch.setenv("TCP_KERNEL", "scalar")
+    wl = W.perf_box(20, thermal="lb_d3q7", ny=16, nz=14, r_min=3.0, r_max=4.0, seed=8)
+    want = run_oracle(wl, 50, extra=PARABOLA)
+    got, _ = run_gpu(wl, 50, extra=PARABOLA, precision="f32")
+    assert_parity_f32(got, want)

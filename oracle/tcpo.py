@@ -132,13 +132,13 @@ _MAX_THREADS = None
 
 
 def threads_for(cells: int) -> int:
-    """One thread per 1024 cells, at most what OpenMP offers.  On the small grids of the pins a parallel region
+    """One thread per 288 cells (a 48 x 24 channel gets 4), at most what OpenMP offers.  On the small grids of the pins a parallel region
     costs more than it saves, and with spinning OpenMP barriers a busy box makes it far worse (measured: 512 cells,
     8 threads, two processes at once: 30-60 ms per step against 12 ms with one thread)."""
     global _MAX_THREADS
     if _MAX_THREADS is None:
         _MAX_THREADS = num_threads()
-    return max(1, min(_MAX_THREADS, cells // 1024))
+    return max(1, min(_MAX_THREADS, cells // 288))
 
 
 class Oracle:

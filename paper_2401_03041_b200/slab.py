@@ -62,6 +62,12 @@ def exchange_faces(send_lo, send_hi, recv_lo, recv_hi, lower, upper, group=None)
     send_hi -> `upper`'s recv_lo, send_lo -> `lower`'s recv_hi.  Receives are posted in the mirrored order of the
     sends, so that with two ranks in a periodic box (lower == upper) the pairs still match up."""
     import torch.distributed as dist
+    # a backend without device-to-device transport (gloo) gets the messages through host memory
+    via_host = dist.get_backend(group) == "gloo" and any(t is not None and t.is_cuda for t in (send_lo, send_hi))
+    dev = (recv_lo, recv_hi)
+    if via_host:
+        host = lambda t: None if t is None else t.cpu()        # synchronises the current stream
+        send_lo, send_hi, recv_lo, recv_hi = host(send_lo), host(send_hi), host(recv_lo), host(recv_hi)
     ops = []
     if upper is not None:
         ops.append(dist.P2POp(dist.isend, send_hi, upper, group))
@@ -74,6 +80,11 @@ def exchange_faces(send_lo, send_hi, recv_lo, recv_hi, lower, upper, group=None)
     if ops:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
+    if via_host:
+        if lower is not None:
+            dev[0].copy_(recv_lo)
+        if upper is not None:
+            dev[1].copy_(recv_hi)
 
 
 def fill_ghost_planes(a_ext, lo, hi, lower, upper, group=None, z_axis=-3):

@@ -205,7 +205,7 @@ def run_ours(args):
     value = aggregate_mlups(N, args.steps, world, ms_max)
     # roofline calibration: the same access pattern and staging with stencils and collisions removed
     pattern_ms = None
-    if rank == 0 and args.streaming == "two_grid":
+    if rank == 0 and args.streaming == "two_grid" and QT[thermal]:   # calibrated for the one-kernel (thermal LB) step only
         sim.pattern_copy_ms(3)
         pattern_ms = sim.pattern_copy_ms(max(5, min(args.steps, 20)))
     phi_chk = sim.read_fields_device()[0]
@@ -336,6 +336,7 @@ def run_slabs(args):
         msg = B.tcp_halo_bytes(s.sim._h)
         desc = f"one z-slab of {n}x{n}x{n} per rank of a {n}x{n}x{n * world} periodic box, NCCL point-to-point"
     else:
+        args.slabs = max(args.slabs, 2)
         box = LocalSlabs(n, n, n, args.slabs, params)
         box.init_fields(wl.phi.to(tdt), None, wl.T.to(tdt))
         launches = lambda: box.launches

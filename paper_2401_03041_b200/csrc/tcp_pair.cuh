@@ -126,7 +126,7 @@ __device__ __forceinline__ void stencil27_pair(const StepArgs<f32x2>& A, const N
 }
 
 template <int QT>
-constexpr int pair_min_blocks() { return QT >= 15 ? 2 : TCP_MINB; }   // same staging footprint as the fp64 kernels
+__host__ __device__ constexpr int pair_min_blocks() { return QT >= 15 ? 2 : TCP_MINB; }   // same staging footprint as the fp64 kernels
 
 template <int QT, bool WALLS, int MODE, int AA>
 __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair_kernel(const StepArgs<f32x2> A) {
@@ -187,6 +187,8 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair
     real u[3];
 #pragma unroll
     for (int al = 0; al < 3; ++al) { const float2 t = *reinterpret_cast<const float2*>(A.u + al * N + cell); u[al] = real(t.x, t.y); }
+
+    prefetch_next_wave<float, QT, AA, StepArgs<f32x2>>(A, 2 * kBlock, pair_min_blocks<QT>());
 
     real phi_new;
     {

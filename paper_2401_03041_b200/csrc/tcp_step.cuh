@@ -327,12 +327,62 @@ __device__ __forceinline__ void cp_async_elem(real* smem_dst, const real* gsrc) 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// L2 prefetch for the next wave of blocks (staged kernels).  The block scheduler hands out blocks in index order, so
+// the blocks about (resident blocks) ahead of this one start one block lifetime from now.  The blocks of a launch are
+// taken in groups of NR = 54 + Q_T + 7 (one per array row the step reads: h, g, f planes, phi and T at z and z + 1,
+// u); block r of a group asks L2, with ONE cp.async.bulk.prefetch (SASS UBLKPF.L2) issued by one thread, for row r
+// of all NR blocks of the group that lies TCP_PF per cent of a wave ahead (NR x cells_per_block consecutive cells,
+// ~70 KB).  The HBM reads of the coming blocks are then in flight while the resident blocks are in their collision
+// phase, and their staged copies find the lines in L2: measured 12.4 -> 11.0 ms per step at 400^3 fp64 D3Q7, best at
+// half a wave (profiles/r01_notes.md section 15; 1.5 waves ahead the lines are evicted again before use and the step
+// slows to 14.6 ms).  A hint only: the segment is addressed without the periodic wrap and clamped into the array.
+#ifndef TCP_PF
+#define TCP_PF 50
+#endif
+template <typename elem, int QT, int AA, typename Args>
+__device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_block, int resident) {
+    if constexpr (TCP_PF > 0) {
+        if (threadIdx.x != 0) return;
+        constexpr int NP = 54 + QT, NR = NP + 7;
+        unsigned nsm;
+        asm("mov.u32 %0, %%nsmid;" : "=r"(nsm));
+        const unsigned r = blockIdx.x % NR;
+        const long long N = A.ncell;
+        const long long c0 = (long long)A.cell0 + (long long)(blockIdx.x - r + NR + (TCP_PF * resident * nsm) / 100) * cells_per_block;
+        if (c0 >= A.cell1) return;
+        const elem* base;
+        int q27i = 13, plane = 0, Q = 27;
+        long long off = c0;
+        if (r < 27) { base = A.h_in; plane = q27i = r; }
+        else if (r < 54) { base = A.g_in; plane = q27i = r - 27; }
+        else if (r < NP) {
+            base = A.f_in; plane = r - 54; Q = QT;
+            static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; if (plane == k) q27i = q_of(QT, k); });
+        } else {
+            const int j = r - NP;
+            if (j < 4) { base = j < 2 ? A.phi_in : A.T_in; if (j & 1) off += (long long)A.nx * A.ny; }
+            else { base = A.u; plane = j - 4; }
+        }
+        if (r < NP) {
+            if (AA != 1) off -= cx27(q27i) + A.nx * (cy27(q27i) + (long long)A.ny * cz27(q27i));
+            if (AA == 2) plane = Q - 1 - plane;
+        }
+        long long len = min((long long)NR * cells_per_block, (long long)A.cell1 - c0) + 2;
+        off = max(0LL, off);
+        len = min(len, N - off);
+        if (len <= 0) return;
+        const unsigned long long addr = (unsigned long long)__cvta_generic_to_global(base + plane * N + off) & ~15ULL;
+        const unsigned bytes = (unsigned)(len * sizeof(elem)) & ~15u;
+        if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(addr), "r"(bytes) : "memory");
+    }
+}
+
 // Residency: (54 + Q_T) x 128 x sizeof(real) bytes of staging per block.  In fp64 three blocks of the
 // D3Q15 / D3Q19 variants would take 212-224 KB of the SM's 256 KB, leaving almost no L1 for the
 // phi / T stencil loads (measured 0.65 of the HBM peak against 0.81-0.84 for D3Q7 and for D3Q27, which
 // only fits two blocks anyway), so those are compiled for two blocks per SM.
 template <typename real, int QT>
-constexpr int async_min_blocks() {
+__host__ __device__ constexpr int async_min_blocks() {
     if (sizeof(real) == 4) return 5;   // fp32: 31 KB of staging per block, <= 102 registers; 5 blocks measured +2.7 % over 4
     return (sizeof(real) == 8 && QT >= 15) ? 2 : TCP_MINB;
 }
@@ -401,6 +451,8 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         stencil27<real, WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
     }
     real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
+
+    if constexpr (MODE != 3) prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT>());
 
     real phi_new;
     {

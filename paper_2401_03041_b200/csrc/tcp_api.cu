@@ -173,14 +173,34 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
 
 unsigned grid_for(size_t n) { return (unsigned)((n + tcp::kBlock - 1) / tcp::kBlock); }
 
+// the z-marching stage kernel is instantiated per (walls, RkArgs::mode, heat source present)
+template <typename real, bool WALLS, int MODE>
+void launch_rk_march_q(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
+    if (R.S.q_src) tcp::rk_stage_march_kernel<real, WALLS, MODE, true><<<grid, block, 0, s->stream>>>(R);
+    else tcp::rk_stage_march_kernel<real, WALLS, MODE, false><<<grid, block, 0, s->stream>>>(R);
+}
+template <typename real, bool WALLS>
+void launch_rk_march_w(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
+    switch (R.mode) {
+    case 0: launch_rk_march_q<real, WALLS, 0>(s, R, grid, block); break;
+    case 1: launch_rk_march_q<real, WALLS, 1>(s, R, grid, block); break;
+    case 2: launch_rk_march_q<real, WALLS, 2>(s, R, grid, block); break;
+    default: launch_rk_march_q<real, WALLS, 3>(s, R, grid, block); break;
+    }
+}
+template <typename real>
+void launch_rk_march(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
+    if (s->walls) launch_rk_march_w<real, true>(s, R, grid, block);
+    else launch_rk_march_w<real, false>(s, R, grid, block);
+}
+
 template <typename real>
 void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
     const int P = s->nx * s->ny, planes = (R.S.cell1 - R.S.cell0) / P;       // whole planes [cell0, cell1)
     if (s->use_async) {   // default: z-marching tile kernel (tcp_rk.cuh)
         const dim3 block(tcp::kRkTX, tcp::kRkTY);
         const dim3 grid((s->nx + tcp::kRkTX - 1) / tcp::kRkTX, (s->ny + tcp::kRkTY - 1) / tcp::kRkTY, (planes + tcp::kRkCZ - 1) / tcp::kRkCZ);
-        if (s->walls) tcp::rk_stage_march_kernel<real, true><<<grid, block, 0, s->stream>>>(R);
-        else tcp::rk_stage_march_kernel<real, false><<<grid, block, 0, s->stream>>>(R);
+        launch_rk_march<real>(s, R, grid, block);
         return;
     }
     const unsigned grid = grid_for((size_t)(R.S.cell1 - R.S.cell0));

@@ -245,11 +245,11 @@ def run_ours(args):
     if QT[thermal]:
         k_ms = kernel_ms / args.steps                      # one fused kernel per step
         achieved = fused_bytes / (k_ms * 1e-3) / 1e9
-        kname = "fused_step_kernel"
+        kname = ("fused_step_pair_kernel" if prec == "f32" and os.environ.get("TCP_KERNEL") != "scalar" else "fused_step_async_kernel")
     else:
         k_ms = kernel_ms / args.steps
         achieved = step_bytes / (k_ms * 1e-3) / 1e9        # whole step (fused kernel + RK stages)
-        kname = "fused_step_kernel + rk_stage_kernel (whole step)"
+        kname = "fused_step_async_kernel + rk_stage_march_kernel (whole step)"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": recorded_traffic(f"{thermal}_{prec}_{n}"), "kernel": kname, "peak_source": peak_src,
                 "algorithmic_bytes_per_cell": (fused_bytes if QT[thermal] else step_bytes) / N,

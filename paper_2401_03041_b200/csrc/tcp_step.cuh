@@ -452,7 +452,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
     }
     real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
 
-    if constexpr (MODE != 3) prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT>());
+    prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT>());
 
     real phi_new;
     {

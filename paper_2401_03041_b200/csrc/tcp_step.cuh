@@ -339,6 +339,9 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 #ifndef TCP_PF
 #define TCP_PF 50
 #endif
+#ifndef TCP_PF2
+#define TCP_PF2 40
+#endif
 template <typename elem, int QT, int AA, typename Args>
 __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_block, int resident) {
     if constexpr (TCP_PF > 0) {
@@ -348,7 +351,8 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
         asm("mov.u32 %0, %%nsmid;" : "=r"(nsm));
         const unsigned r = blockIdx.x % NR;
         const long long N = A.ncell;
-        const long long c0 = (long long)A.cell0 + (long long)(blockIdx.x - r + NR + (TCP_PF * resident * nsm) / 100) * cells_per_block;
+        const int pf = resident == 2 ? TCP_PF2 : TCP_PF;   // kernels with two blocks per SM: the optimum is flatter and earlier
+        const long long c0 = (long long)A.cell0 + (long long)(blockIdx.x - r + NR + (pf * resident * nsm) / 100) * cells_per_block;
         if (c0 >= A.cell1) return;
         const elem* base;
         int q27i = 13, plane = 0, Q = 27;

@@ -334,7 +334,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // of all NR blocks of the group that lies TCP_PF per cent of a wave ahead (NR x cells_per_block consecutive cells,
 // ~70 KB).  The HBM reads of the coming blocks are then in flight while the resident blocks are in their collision
 // phase, and their staged copies find the lines in L2: measured 12.4 -> 11.0 ms per step at 400^3 fp64 D3Q7, best at
-// half a wave (profiles/r01_notes.md section 15; 1.5 waves ahead the lines are evicted again before use and the step
+// half a wave, 40 % for the kernels with two blocks per SM (profiles/r01_notes.md section 15; 1.5 waves ahead the lines are evicted again before use and the step
 // slows to 14.6 ms).  A hint only: the segment is addressed without the periodic wrap and clamped into the array.
 #ifndef TCP_PF
 #define TCP_PF 50

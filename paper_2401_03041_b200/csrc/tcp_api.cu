@@ -129,6 +129,15 @@ namespace {
 
 template <typename real> real* ptr(const tcp_sim* s, size_t off) { return reinterpret_cast<real*>(s->base + off); }
 
+// constants {m, s1, s2} of tcp::fast_div for the divisor d >= 1
+void fast_div_make(unsigned d, unsigned c[3]) {
+    unsigned l = 0;
+    while ((1ull << l) < d) ++l;                       // l = ceil(log2 d)
+    c[0] = (unsigned)(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+    c[1] = l < 1 ? l : 1;
+    c[2] = l > 1 ? l - 1 : 0;
+}
+
 template <typename real>
 tcp::StepArgs<real> make_args(const tcp_sim* s) {
     tcp::StepArgs<real> A;
@@ -151,6 +160,9 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     A.rho_L = (real)P.rho_L; A.drho = (real)(P.rho_H - P.rho_L);
     A.tau_L = (real)P.tau_L; A.dtau = (real)(P.tau_H - P.tau_L);
     A.xi = (real)P.xi; A.w_phi = (real)(1.0 / (0.5 + 3.0 * P.M));
+    A.inv_xi = (real)(1.0 / P.xi);
+    fast_div_make((unsigned)s->nx, A.div_nx);
+    fast_div_make((unsigned)s->ny, A.div_ny);
     A.sigma_ref = (real)P.sigma_ref; A.sigma_T = (real)P.sigma_T; A.T_ref = (real)P.T_ref; A.sigma_TT = (real)P.sigma_TT;
     A.kappa_L = (real)P.kappa_L; A.dkappa = (real)(P.kappa_H - P.kappa_L);
     A.cp_L = (real)P.cp_L; A.dcp = (real)(P.cp_H - P.cp_L);

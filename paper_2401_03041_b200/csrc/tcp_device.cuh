@@ -28,6 +28,8 @@ struct StepArgs {
     const real* wallT[3][2];         // wall-temperature planes
     real rho_L, drho, tau_L, dtau;   // eqs. 14, 22
     real xi, w_phi;                  // eq. 15; rate 1/(1/2 + 3M) (eq. 11, reading G3)
+    real inv_xi;                     // 1 / xi (host-computed: two fp64 divisions per cell less)
+    unsigned div_nx[3], div_ny[3];   // cell -> (x, y, z) without integer division: fast_div constants {m, s1, s2}
     real sigma_ref, sigma_T, T_ref;  // eq. 9
     real sigma_TT;                   // parabolic sigma(T) (reading S19); 0 = eq. 9
     real kappa_L, dkappa, cp_L, dcp; // eqs. 23-24 (reading G5)
@@ -55,6 +57,8 @@ struct StepArgs<f32x2> {
     const float* wallT[3][2];
     f32x2 rho_L, drho, tau_L, dtau;
     f32x2 xi, w_phi;
+    f32x2 inv_xi;
+    unsigned div_nx[3], div_ny[3];
     f32x2 sigma_ref, sigma_T, T_ref;
     f32x2 sigma_TT;
     f32x2 kappa_L, dkappa, cp_L, dcp;
@@ -65,9 +69,10 @@ struct StepArgs<f32x2> {
     __host__ explicit StepArgs(const StepArgs<float>& A)
         : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), cell0(A.cell0), cell1(A.cell1), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
           f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src),
-          rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), sigma_ref(A.sigma_ref),
+          rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), inv_xi(A.inv_xi), sigma_ref(A.sigma_ref),
           sigma_T(A.sigma_T), T_ref(A.T_ref), sigma_TT(A.sigma_TT), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
           s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving) {
+        for (int k = 0; k < 3; ++k) { div_nx[k] = A.div_nx[k]; div_ny[k] = A.div_ny[k]; }
         for (int a = 0; a < 3; ++a) {
             wall[a] = A.wall[a];
             grav[a] = f32x2(A.grav[a]);
@@ -83,6 +88,14 @@ struct StepArgs<f32x2> {
 // neighbourhood of one cell: element offsets to the 26 neighbours with periodic wrap, or, on a
 // WALLS axis, clamped to the mirror cell (reading S9: walls half a cell outside the end cells)
 
+// n / d for any 32-bit n, d >= 1 fixed per launch (Granlund-Montgomery round-up method): with l = ceil(log2 d),
+// m = floor(2^32 (2^l - d) / d) + 1, s1 = min(l, 1), s2 = max(l - 1, 0):  q = (t + ((n - t) >> s1)) >> s2, t = mulhi(m, n).
+// c = {m, s1, s2} comes from the host (fast_div_make in tcp_api.cu).
+__device__ __forceinline__ unsigned fast_div(unsigned n, const unsigned c[3]) {
+    const unsigned t = __umulhi(c[0], n);
+    return (t + ((n - t) >> c[1])) >> c[2];
+}
+
 template <bool WALLS>
 struct Nbh {
     int idx;
@@ -94,9 +107,9 @@ struct Nbh {
     // thread id -> cell: plain x, y, z order (a z-slab visiting order was measured 2-3 % slower, profiles/r01_notes.md)
     template <typename real>
     __device__ __forceinline__ void init(const StepArgs<real>& A, int cell) {
-        const int x = cell % A.nx;
-        const int t = cell / A.nx;
-        init_xyz(A, x, t % A.ny, t / A.ny);
+        const int t = (int)fast_div((unsigned)cell, A.div_nx), x = cell - t * A.nx;
+        const int z = (int)fast_div((unsigned)t, A.div_ny), y = t - z * A.ny;
+        init_xyz(A, x, y, z);
     }
     template <typename real>
     __device__ __forceinline__ void init_xyz(const StepArgs<real>& A, int x, int y, int z) {

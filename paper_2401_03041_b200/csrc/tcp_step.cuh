@@ -81,7 +81,7 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
     if constexpr (real_traits<real>::single) { phin_exact = exact_sum27<real>(h); phin = narrow<real>(phin_exact); }
     // a = c_s^2 [4 phi (1 - phi) / xi] n,  n = G / sqrt(G.G + eps)   (eq. 15, readings S7, S8)
     const real inv = rsqrt_<real>(G[0] * G[0] + G[1] * G[1] + G[2] * G[2] + A.eps);
-    const real mag = real(4.0 / 3.0) * phi_c * (real(1) - phi_c) / A.xi * inv;
+    const real mag = real(4.0 / 3.0) * phi_c * (real(1) - phi_c) * A.inv_xi * inv;
     real a[3] = {mag * G[0], mag * G[1], mag * G[2]};
     const real w = A.w_phi;
     if (MODE == 1) {   // a~ = (1-w) a + w [a_eq + F(a (2-w)/w)/2]
@@ -130,7 +130,7 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
     const real dsigma = A.sigma_T + A.sigma_TT * dTr;
     const real sigma = A.sigma_ref + A.sigma_T * dTr + real(0.5) * A.sigma_TT * dTr * dTr;
     // mu_phi = 4 beta phi (phi-1)(phi-1/2) - k lap phi, beta = 12 sigma/xi, k = 3 sigma xi/2  (S5)
-    const real mu = real(48) * sigma / A.xi * phi_c * (phi_c - real(1)) * (phi_c - real(0.5)) - real(1.5) * sigma * A.xi * lapPhi;
+    const real mu = real(48) * sigma * A.inv_xi * phi_c * (phi_c - real(1)) * (phi_c - real(0.5)) - real(1.5) * sigma * A.xi * lapPhi;
     const real GG = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
     const real TG = Th[0] * G[0] + Th[1] * G[1] + Th[2] * G[2];
     const real mar = real(1.5) * A.xi * dsigma;             // eq. 8 (with |grad phi|^2, G2)
@@ -430,6 +430,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         return wall_link ? base + (Q - 1 - k) * N + cell : base + k * N + nb.at(cx, cy, cz);
     };
 
+    real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
 #pragma unroll
     for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + q * kBlock + tid, src_of(A.h_in, 27, q, q));
     cp_async_commit();
@@ -446,7 +447,6 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
 
     // MODE 3 is a roofline calibration, not a step of the method: same pulls, staging and stores, but the
     // stencils and collisions are left out (h, g, f are streamed unchanged; phi, T, u copied through).
-    real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
     if constexpr (MODE == 3) {
         phi_c = A.phi_in[cell]; T_c = A.T_in[cell];
         G[0] = G[1] = G[2] = Th[0] = Th[1] = Th[2] = lapPhi = lapT = real(0);

@@ -163,6 +163,7 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
     A.inv_xi = (real)(1.0 / P.xi);
     fast_div_make((unsigned)s->nx, A.div_nx);
     fast_div_make((unsigned)s->ny, A.div_ny);
+    fast_div_make((unsigned)(s->nx > 1 ? s->nx / 2 : 1), A.div_hx);
     A.sigma_ref = (real)P.sigma_ref; A.sigma_T = (real)P.sigma_T; A.T_ref = (real)P.T_ref; A.sigma_TT = (real)P.sigma_TT;
     A.kappa_L = (real)P.kappa_L; A.dkappa = (real)(P.kappa_H - P.kappa_L);
     A.cp_L = (real)P.cp_L; A.dcp = (real)(P.cp_H - P.cp_L);

@@ -30,6 +30,7 @@ struct StepArgs {
     real xi, w_phi;                  // eq. 15; rate 1/(1/2 + 3M) (eq. 11, reading G3)
     real inv_xi;                     // 1 / xi (host-computed: two fp64 divisions per cell less)
     unsigned div_nx[3], div_ny[3];   // cell -> (x, y, z) without integer division: fast_div constants {m, s1, s2}
+    unsigned div_hx[3];              // the same for nx / 2 (pair kernel)
     real sigma_ref, sigma_T, T_ref;  // eq. 9
     real sigma_TT;                   // parabolic sigma(T) (reading S19); 0 = eq. 9
     real kappa_L, dkappa, cp_L, dcp; // eqs. 23-24 (reading G5)
@@ -58,7 +59,7 @@ struct StepArgs<f32x2> {
     f32x2 rho_L, drho, tau_L, dtau;
     f32x2 xi, w_phi;
     f32x2 inv_xi;
-    unsigned div_nx[3], div_ny[3];
+    unsigned div_nx[3], div_ny[3], div_hx[3];
     f32x2 sigma_ref, sigma_T, T_ref;
     f32x2 sigma_TT;
     f32x2 kappa_L, dkappa, cp_L, dcp;
@@ -72,7 +73,7 @@ struct StepArgs<f32x2> {
           rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), inv_xi(A.inv_xi), sigma_ref(A.sigma_ref),
           sigma_T(A.sigma_T), T_ref(A.T_ref), sigma_TT(A.sigma_TT), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
           s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving) {
-        for (int k = 0; k < 3; ++k) { div_nx[k] = A.div_nx[k]; div_ny[k] = A.div_ny[k]; }
+        for (int k = 0; k < 3; ++k) { div_nx[k] = A.div_nx[k]; div_ny[k] = A.div_ny[k]; div_hx[k] = A.div_hx[k]; }
         for (int a = 0; a < 3; ++a) {
             wall[a] = A.wall[a];
             grav[a] = f32x2(A.grav[a]);

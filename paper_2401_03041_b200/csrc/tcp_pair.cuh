@@ -24,9 +24,9 @@ struct NbhPair {
     __device__ __forceinline__ void init(const StepArgs<f32x2>& A, int pair) {
         nx = A.nx; ny = A.ny;
         const int hx = A.nx >> 1;
-        x = 2 * (pair % hx);
-        const int t = pair / hx;
-        const int y = t % A.ny, z = t / A.ny;
+        const int t = (int)fast_div((unsigned)pair, A.div_hx);
+        x = 2 * (pair - t * hx);
+        const int z = (int)fast_div((unsigned)t, A.div_ny), y = t - z * A.ny;
         const int sy = A.nx, sz = A.nx * A.ny;
         idx = x + sy * y + sz * z;
         xm1 = x > 0 ? -1 : A.nx - 1;

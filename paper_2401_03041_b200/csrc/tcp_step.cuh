@@ -456,7 +456,8 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
     }
     real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
 
-    prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT>());
+    // (not in the calibration kernel: without arithmetic its blocks are too short-lived, measured 10.98 ms with against 10.5 ms without)
+    if constexpr (MODE != 3) prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT>());
 
     real phi_new;
     {

@@ -189,8 +189,14 @@ unsigned grid_for(size_t n) { return (unsigned)((n + tcp::kBlock - 1) / tcp::kBl
 // the z-marching stage kernel is instantiated per (walls, RkArgs::mode, heat source present)
 template <typename real, bool WALLS, int MODE>
 void launch_rk_march_q(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
-    if (R.S.q_src) tcp::rk_stage_march_kernel<real, WALLS, MODE, true><<<grid, block, 0, s->stream>>>(R);
-    else tcp::rk_stage_march_kernel<real, WALLS, MODE, false><<<grid, block, 0, s->stream>>>(R);
+    const bool dk = s->P.kappa_H != s->P.kappa_L;       // grad kappa . grad T present
+    if (R.S.q_src) {
+        if (dk) tcp::rk_stage_march_kernel<real, WALLS, MODE, true, true><<<grid, block, 0, s->stream>>>(R);
+        else tcp::rk_stage_march_kernel<real, WALLS, MODE, true, false><<<grid, block, 0, s->stream>>>(R);
+    } else {
+        if (dk) tcp::rk_stage_march_kernel<real, WALLS, MODE, false, true><<<grid, block, 0, s->stream>>>(R);
+        else tcp::rk_stage_march_kernel<real, WALLS, MODE, false, false><<<grid, block, 0, s->stream>>>(R);
+    }
 }
 template <typename real, bool WALLS>
 void launch_rk_march_w(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {

@@ -28,7 +28,9 @@ struct Plane3 {          // in-plane reductions of one field on one z plane
 // MODE = RkArgs::mode and HAS_Q = (q_src != nullptr) are compile-time here, and the plane loop is unrolled three
 // times so that the three-plane register window (z-1, z, z+1) rotates by renaming instead of by moves: 273 -> 2xx
 // instructions per cell (ncu: the kernel keeps the issue slots 54 % busy, so instructions are what it is made of).
-template <typename real, bool WALLS, int MODE, bool HAS_Q>
+// HAS_DK = (kappa_H != kappa_L): with equal conductivities grad kappa . grad T of eq. 4 vanishes identically, so the
+// phi tile, its nine shared loads and its reductions are left out and phi is read at the cell only (for rho c_p).
+template <typename real, bool WALLS, int MODE, bool HAS_Q, bool HAS_DK>
 __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage_march_kernel(const RkArgs<real> R) {
     const StepArgs<real>& A = R.S;
     constexpr int TX = kRkTX, TY = kRkTY, PX = TX + 2, PY = TY + 2, PE = PX * PY;
@@ -73,7 +75,7 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage
             if (!e_on[i]) continue;
             const int idx = e_idx2d[i] + sz * Z;
             real vy = __ldg(R.Y + idx);
-            pfP[i] = __ldg(A.phi_in + idx);
+            if (HAS_DK) pfP[i] = __ldg(A.phi_in + idx);
             if (WALLS) {   // Dirichlet ghost 2 T_w - Y(mirror); first crossed axis in x, y, z order (S9, S17)
                 if (e_fx[i] >= 0) vy = real(2) * A.wallT[0][e_fx[i]][Z * A.ny + e_tang_y[i]] - vy;
                 else if (e_fy[i] >= 0) vy = real(2) * A.wallT[1][e_fy[i]][Z * A.nx + e_tang_x[i]] - vy;
@@ -85,7 +87,7 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage
     auto store_plane = [&](int buf) {
 #pragma unroll
         for (int i = 0; i < NE; ++i)
-            if (e_on[i]) { tileY[buf][tid + i * TX * TY] = pfY[i]; tileP[buf][tid + i * TX * TY] = pfP[i]; }
+            if (e_on[i]) { tileY[buf][tid + i * TX * TY] = pfY[i]; if (HAS_DK) tileP[buf][tid + i * TX * TY] = pfP[i]; }
     };
     const real c16 = real(1.0 / 6.0), c23 = real(2.0 / 3.0), half = real(0.5);
     auto reduce_plane = [&](const real* t) {
@@ -111,11 +113,11 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage
     fetch_plane(z0); store_plane(1);
     fetch_plane(z0 + 1);                   // stays in registers until iteration 0 stores it
     __syncthreads();
-    Ym = reduce_plane(tileY[0]); Pm = reduce_plane(tileP[0]);
-    Yc = reduce_plane(tileY[1]); Pc = reduce_plane(tileP[1]);
+    Ym = reduce_plane(tileY[0]); Yc = reduce_plane(tileY[1]);
+    if (HAS_DK) { Pm = reduce_plane(tileP[0]); Pc = reduce_plane(tileP[1]); }
     __syncthreads();                       // buffer 0 may now be overwritten
     // cell data (u, T^n, accumulator, source) of plane z0 + k are requested one iteration ahead as well
-    real nu[3] = {real(0), real(0), real(0)}, nTn = real(0), nacc = real(0), nq = real(0);
+    real nu[3] = {real(0), real(0), real(0)}, nTn = real(0), nacc = real(0), nq = real(0), nphi = real(0);
     auto fetch_cell = [&](int zz) {
         if (!inside) return;
         const int c = x + sy * y + sz * zz;
@@ -123,6 +125,7 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage
         nTn = R.Tn[c];
         if (MODE >= 2) nacc = R.acc_in[c];
         if (HAS_Q) nq = A.q_src[c];
+        if (!HAS_DK) nphi = A.phi_in[c];
     };
     fetch_cell(z0);
     const real c_out = R.c_out, c_acc = R.c_acc;
@@ -131,26 +134,29 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage
                      const Plane3<real>& Pm, const Plane3<real>& Pc, Plane3<real>& Pp) {
         const int buf = k & 1;
         const int cell = x + sy * y + sz * (z0 + k);
-        const real u[3] = {nu[0], nu[1], nu[2]}, Tn = nTn, acc = nacc, qT = nq;
+        const real u[3] = {nu[0], nu[1], nu[2]}, Tn = nTn, acc = nacc, qT = nq, phi_here = nphi;
         if (k + 1 < nzc) fetch_cell(z0 + k + 1);
         store_plane(buf);                          // plane z0 + k + 1
         if (k + 1 < nzc) fetch_plane(z0 + k + 2);  // next one: its latency hides behind this iteration
         __syncthreads();
-        Yp = reduce_plane(tileY[buf]); Pp = reduce_plane(tileP[buf]);
+        Yp = reduce_plane(tileY[buf]);
+        if (HAS_DK) Pp = reduce_plane(tileP[buf]);
         if (inside) {
-            real gY[3], G[3];
+            real gY[3], G[3] = {real(0), real(0), real(0)};
             gY[0] = (Ym.Dx + Yp.Dx) * c16 + Yc.Dx * c23;
             gY[1] = (Ym.Dy + Yp.Dy) * c16 + Yc.Dy * c23;
             gY[2] = (Yp.S - Ym.S) * half;
             const real lapY = real(6) * (((Ym.S + Yp.S) * c16 + Yc.S * c23) - Yc.c);
-            G[0] = (Pm.Dx + Pp.Dx) * c16 + Pc.Dx * c23;
-            G[1] = (Pm.Dy + Pp.Dy) * c16 + Pc.Dy * c23;
-            G[2] = (Pp.S - Pm.S) * half;
-            const real phi_c = Pc.c;
+            if (HAS_DK) {
+                G[0] = (Pm.Dx + Pp.Dx) * c16 + Pc.Dx * c23;
+                G[1] = (Pm.Dy + Pp.Dy) * c16 + Pc.Dy * c23;
+                G[2] = (Pp.S - Pm.S) * half;
+            }
+            const real phi_c = HAS_DK ? Pc.c : phi_here;
             const real kap = A.kappa_L + phi_c * A.dkappa;
             const real rcp = (A.rho_L + phi_c * A.drho) * (A.cp_L + phi_c * A.dcp);
             const real adv = u[0] * gY[0] + u[1] * gY[1] + u[2] * gY[2];
-            const real dk = A.dkappa * (G[0] * gY[0] + G[1] * gY[1] + G[2] * gY[2]);
+            const real dk = HAS_DK ? A.dkappa * (G[0] * gY[0] + G[1] * gY[1] + G[2] * gY[2]) : real(0);
             const real rhs = -adv + (dk + kap * lapY) / rcp + qT;
             if (MODE == 3) {
                 R.out[cell] = acc + c_acc * rhs;

@@ -116,7 +116,10 @@ int tcp_relax_temperature(tcp_sim *s, int nsteps);
  * A step has `tcp_halo_phases` phases, each followed by one message per face: 1 on the thermal LB paths (the
  * fused kernel; message [9 h~ planes][9 g~ planes][1, 5, 5 or 9 f~ planes][phi][T], nx*ny values each), 3 / 5 on
  * the RK2 / RK4 paths (Algorithm 2: the fused phase + hydro kernel with message [9 h~][9 g~][phi], then every
- * Runge-Kutta stage with its output plane as message, because the next stage differentiates it).
+ * Runge-Kutta stage with its output plane as message, because the next stage differentiates it).  With
+ * kappa_H = kappa_L the first stage runs inside the fused kernel (grad kappa . grad T vanishes and everything else
+ * it needs is already in the cell's thread): one phase less (2 / 4), and the first message also carries the
+ * plane of the first stage's output ([9 h~][9 g~][phi][Y1]).
  * `tcp_halo_message_bytes` gives the size of a phase's message, `tcp_halo_bytes` that of the largest (phase 0).
  * `send_*` / `recv_*` are caller-owned DEVICE buffers of tcp_halo_bytes (NULL for a face without ghost plane);
  * `comm_stream` is the caller's cudaStream_t on which the library gathers and scatters and on which the caller

@@ -262,12 +262,32 @@ int rk_stages(const tcp_sim* s, const tcp::StepArgs<real>& A, const real* phi, t
     return 4;
 }
 
+// Stage 1 inside the fused kernel (rk_stage1_local, tcp_step.cuh): the Runge-Kutta paths with equal conductivities,
+// whenever a staged kernel runs the step (the register-staged A/B kernel of TCP_KERNEL=flat keeps the separate stage).
+bool rk_first_stage_fused(const tcp_sim* s) {
+    const int th = s->P.thermal;
+    if (th != TCP_THERMAL_RK2 && th != TCP_THERMAL_RK4) return false;
+    if (s->P.kappa_H != s->P.kappa_L) return false;
+    const bool flat = !s->use_async && !s->P.high_rate_equals_shear && s->P.s_high == 1.0 && s->P.streaming == TCP_STREAM_TWO_GRID;
+    return !flat;
+}
+
+// stages [first, n) of the Runge-Kutta update
 template <typename real>
-void rk_update(tcp_sim* s, const tcp::StepArgs<real>& A, const real* phi) {
+void rk_update(tcp_sim* s, const tcp::StepArgs<real>& A, const real* phi, int first = 0) {
     tcp::RkArgs<real> st[4];
     const int n = rk_stages<real>(s, A, phi, st);
-    for (int i = 0; i < n; ++i) launch_rk_stage<real>(s, st[i]);
-    s->launches += n;
+    for (int i = first; i < n; ++i) launch_rk_stage<real>(s, st[i]);
+    s->launches += n > first ? n - first : 0;
+}
+
+// hand the fused kernel the outputs of stage 1 (Y1, and the RK4 accumulator)
+template <typename real>
+void attach_first_stage(tcp_sim* s, tcp::StepArgs<real>& A) {
+    tcp::RkArgs<real> st[4];
+    if (rk_stages<real>(s, A, A.phi_out, st) == 0) return;
+    A.rk1_out = st[0].out; A.rk1_c_out = st[0].c_out;
+    A.rk1_acc = st[0].mode == 1 ? st[0].acc_out : nullptr; A.rk1_c_acc = st[0].c_acc;
 }
 
 // temperature update alone, phi / u / h~ / g~ frozen
@@ -319,9 +339,12 @@ int launch_fused(tcp_sim* s, const tcp::StepArgs<real>& A) {
 template <typename real>
 int step_once(tcp_sim* s) {
     tcp::StepArgs<real> A = make_args<real>(s);
+    const bool fused1 = rk_first_stage_fused(s);
+    if (fused1) attach_first_stage<real>(s, A);
     int rc = launch_fused<real>(s, A);
     if (rc) return rc;
-    rk_update<real>(s, A, A.phi_out);        // phi^{n+1}; u already holds u^{n+1}
+    A.rk1_out = nullptr; A.rk1_acc = nullptr;
+    rk_update<real>(s, A, A.phi_out, fused1 ? 1 : 0);        // phi^{n+1}; u already holds u^{n+1}
     s->cur = 1 - s->cur;
     s->curT = 1 - s->curT;
     if (s->aa_next) s->aa_next = 3 - s->aa_next;
@@ -334,7 +357,8 @@ int step_once(tcp_sim* s) {
 // (fused phase + hydro kernel, then every stage: its output is differentiated by the next one) ------------
 
 int halo_phases(const tcp_sim* s) {
-    return s->P.thermal == TCP_THERMAL_RK2 ? 3 : (s->P.thermal == TCP_THERMAL_RK4 ? 5 : 1);
+    const int stages = s->P.thermal == TCP_THERMAL_RK2 ? 2 : (s->P.thermal == TCP_THERMAL_RK4 ? 4 : 0);
+    return 1 + stages - (rk_first_stage_fused(s) ? 1 : 0);
 }
 
 // The arrays (pointers to their plane z = 0) of which one z-plane travels in direction dir (+1 up, -1 down)
@@ -344,10 +368,11 @@ int phase_message(const tcp_sim* s, int p, int dir, real* fields[32]) {
     const size_t N = s->N;
     const int o = 1 - s->cur, oT = 1 - s->curT;
     int m = 0;
+    const int f1 = rk_first_stage_fused(s) ? 1 : 0;
     if (p > 0) {
         tcp::RkArgs<real> st[4];
         rk_stages<real>(s, make_args<real>(s), nullptr, st);
-        fields[m++] = st[p - 1].out;
+        fields[m++] = st[p - 1 + f1].out;
         return m;
     }
     for (int q = 0; q < 27; ++q)
@@ -359,6 +384,11 @@ int phase_message(const tcp_sim* s, int p, int dir, real* fields[32]) {
         if (tcp::cz27(tcp::q_of(QT, k)) == dir) fields[m++] = ptr<real>(s, s->L.f[oT]) + k * N;
     fields[m++] = ptr<real>(s, s->L.phi[o]);
     if (QT) fields[m++] = ptr<real>(s, s->L.T[oT]);
+    if (f1) {   // stage 1 ran inside the fused kernel: its output travels with this message
+        tcp::RkArgs<real> st[4];
+        rk_stages<real>(s, make_args<real>(s), nullptr, st);
+        fields[m++] = st[0].out;
+    }
     return m;
 }
 
@@ -396,10 +426,16 @@ int phase_begin(tcp_sim* s, int p) {
     auto planes = [&](int z0, int z1) {       // run the phase on the planes z0..z1
         if (z1 < z0) return (int)TCP_OK;
         A.cell0 = z0 * P; A.cell1 = (z1 + 1) * P;
-        if (p == 0) return launch_fused<real>(s, A);
+        const int f1 = rk_first_stage_fused(s) ? 1 : 0;
+        if (p == 0) {
+            if (f1) attach_first_stage<real>(s, A);
+            const int r = launch_fused<real>(s, A);
+            A.rk1_out = nullptr; A.rk1_acc = nullptr;
+            return r;
+        }
         tcp::RkArgs<real> st[4];
         rk_stages<real>(s, A, A.phi_out, st);
-        launch_rk_stage<real>(s, st[p - 1]);
+        launch_rk_stage<real>(s, st[p - 1 + f1]);
         s->launches++;
         return (int)TCP_OK;
     };
@@ -701,7 +737,7 @@ int tcp_halo_message_bytes(const tcp_sim* s, int phase, size_t* bytes) {
     if (!s || !bytes) return fail(TCP_EINVAL, "NULL argument");
     if (phase < 0 || phase >= halo_phases(s)) return fail(TCP_EINVAL, "phase out of range (tcp_halo_phases)");
     const int QT = thermal_q(s->P.thermal);
-    const size_t planes = phase > 0 ? 1 : 9 + 9 + (size_t)tcp::halo_crossing(QT, 1) + 1 + (QT ? 1 : 0);
+    const size_t planes = phase > 0 ? 1 : 9 + 9 + (size_t)tcp::halo_crossing(QT, 1) + 1 + (QT ? 1 : 0) + (rk_first_stage_fused(s) ? 1 : 0);
     *bytes = planes * s->nx * s->ny * (s->P.precision == TCP_F64 ? 8 : 4);
     return TCP_OK;
 }

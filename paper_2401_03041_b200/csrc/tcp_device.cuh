@@ -25,6 +25,8 @@ struct StepArgs {
     const real* T_in;  real* T_out;
     real* u;                         // [3][N], updated in place (only read locally)
     const real* q_src;               // heat source or nullptr
+    real* rk1_out; real* rk1_acc;    // Runge-Kutta paths with kappa_H = kappa_L: the fused kernel also does stage 1 (tcp_step.cuh,
+    real rk1_c_out, rk1_c_acc;       // rk_stage1_local): Y1 = T^n + c_out R, accumulator = T^n + c_acc R (RK4); nullptr = off
     const real* wallT[3][2];         // wall-temperature planes
     real rho_L, drho, tau_L, dtau;   // eqs. 14, 22
     real xi, w_phi;                  // eq. 15; rate 1/(1/2 + 3M) (eq. 11, reading G3)
@@ -55,6 +57,8 @@ struct StepArgs<f32x2> {
     const float* T_in;  float* T_out;
     float* u;
     const float* q_src;
+    float* rk1_out; float* rk1_acc;
+    f32x2 rk1_c_out, rk1_c_acc;
     const float* wallT[3][2];
     f32x2 rho_L, drho, tau_L, dtau;
     f32x2 xi, w_phi;
@@ -69,7 +73,7 @@ struct StepArgs<f32x2> {
     float wall_u[3][2][3];
     __host__ explicit StepArgs(const StepArgs<float>& A)
         : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), cell0(A.cell0), cell1(A.cell1), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
-          f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src),
+          f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src), rk1_out(A.rk1_out), rk1_acc(A.rk1_acc), rk1_c_out(A.rk1_c_out), rk1_c_acc(A.rk1_c_acc),
           rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), inv_xi(A.inv_xi), sigma_ref(A.sigma_ref),
           sigma_T(A.sigma_T), T_ref(A.T_ref), sigma_TT(A.sigma_TT), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
           s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving) {

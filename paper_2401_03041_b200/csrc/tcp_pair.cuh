@@ -226,6 +226,15 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair
             for (int al = 0; al < 3; ++al) *reinterpret_cast<float2*>(A.u + al * N + cell) = u[al].v;
         }
     }
+    if constexpr (QT == 0) {
+        if (A.rk1_out && active) {   // Runge-Kutta stage 1 of both cells (rk_stage1_local, tcp_step.cuh)
+            real qT(0.0f);
+            if (A.q_src) { const float2 t = *reinterpret_cast<const float2*>(A.q_src + cell); qT = real(t.x, t.y); }
+            const real rhs = rk_stage1_local<real>(A, phi_new, u, Th, lapT, qT);
+            *reinterpret_cast<float2*>(A.rk1_out + cell) = (T_c + A.rk1_c_out * rhs).v;
+            if (A.rk1_acc) *reinterpret_cast<float2*>(A.rk1_acc + cell) = (T_c + A.rk1_c_acc * rhs).v;
+        }
+    }
     if constexpr (QT > 0) {
         cp_async_wait<0>();
         real f[QT];

@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage
         if (!inside) return;
         const int c = x + sy * y + sz * zz;
         nu[0] = A.u[c]; nu[1] = A.u[N + c]; nu[2] = A.u[2 * N + c];
-        nTn = R.Tn[c];
+        if (MODE != 3) nTn = R.Tn[c];             // the last RK4 stage adds to the accumulator only
         if (MODE >= 2) nacc = R.acc_in[c];
         if (HAS_Q) nq = A.q_src[c];
         if (!HAS_DK) nphi = A.phi_in[c];

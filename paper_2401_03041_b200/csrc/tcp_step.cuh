@@ -263,6 +263,19 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
     return Tn;
 }
 
+// ---- Runge-Kutta stage 1 inside the fused kernel (eqs. 4, 25-26) ------------------------------------
+// With kappa_H = kappa_L the term grad kappa . grad T of eq. 4 vanishes and R(T^n) needs nothing beyond what the cell's
+// thread already holds: grad T^n and lap T^n (computed for the Marangoni force), u^{n+1}, phi^{n+1}.  The first stage
+// then costs one or two stores instead of a kernel that re-reads T^n, phi^{n+1} and u^{n+1} (56-64 B per cell).
+// Same expression as rk_stage_march_kernel with dk = 0.
+template <typename real>
+__device__ __forceinline__ real rk_stage1_local(const StepArgs<real>& A, real phi_new, const real u[3], const real Th[3], real lapT, real qT) {
+    const real kap = A.kappa_L + phi_new * A.dkappa;
+    const real rcp = (A.rho_L + phi_new * A.drho) * (A.cp_L + phi_new * A.dcp);
+    const real adv = u[0] * Th[0] + u[1] * Th[1] + u[2] * Th[2];
+    return -adv + (kap * lapT) / rcp + qT;
+}
+
 // ---------------------------------------------------------------------------------------------
 template <typename real, int QT, bool WALLS, int MODE>
 __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const StepArgs<real> A) {
@@ -298,6 +311,13 @@ __global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const Step
 #pragma unroll
         for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
         A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
+    }
+    if constexpr (QT == 0) {
+        if (A.rk1_out) {
+            const real rhs = rk_stage1_local<real>(A, phi_new, u, Th, lapT, A.q_src ? A.q_src[cell] : real(0));
+            A.rk1_out[cell] = T_c + A.rk1_c_out * rhs;
+            if (A.rk1_acc) A.rk1_acc[cell] = T_c + A.rk1_c_acc * rhs;
+        }
     }
     if constexpr (QT > 0) {
         real f[QT];
@@ -491,6 +511,13 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
                 *dst = (WALLS && wl) ? g[q] + wall_velocity_term<real, WALLS>(A, nb, 26 - q) : g[q];
             }
             A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
+        }
+    }
+    if constexpr (QT == 0 && MODE != 3) {
+        if (A.rk1_out && active) {
+            const real rhs = rk_stage1_local<real>(A, phi_new, u, Th, lapT, A.q_src ? A.q_src[cell] : real(0));
+            A.rk1_out[cell] = T_c + A.rk1_c_out * rhs;
+            if (A.rk1_acc) A.rk1_acc[cell] = T_c + A.rk1_c_acc * rhs;
         }
     }
     if constexpr (QT > 0) {

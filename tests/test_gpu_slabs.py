@@ -129,10 +129,23 @@ def test_runge_kutta_tweezer_walls_in_z():
 
 def test_runge_kutta_phases_and_messages():
     wl = configs.perf_box(16, thermal="rk4", ny=12, nz=12, seed=1, r_min=3.0, r_max=4.0)
+    plane = 16 * 12 * 8
+    # equal conductivities (the benchmark fluid): stage 1 runs inside the fused kernel, its output travels with phase 0
+    box = LocalSlabs(16, 12, 12, 2, dict(wl.params))
+    h = box.slabs[0].sim._h
+    assert wl.params["kappa_H"] == wl.params["kappa_L"]
+    assert B.tcp_halo_phases(h) == 4
+    assert [B.tcp_halo_message_bytes(h, p) for p in range(4)] == [20 * plane] + [plane] * 3
+    assert B.tcp_halo_bytes(h) == 20 * plane
+    box.close()
+    box = LocalSlabs(16, 12, 12, 2, dict(wl.params, thermal="rk2"))
+    assert B.tcp_halo_phases(box.slabs[0].sim._h) == 2
+    box.close()
+    # different conductivities: every stage is a kernel of its own
+    wl.params["kappa_H"] = 0.1
     box = LocalSlabs(16, 12, 12, 2, dict(wl.params))
     h = box.slabs[0].sim._h
     assert B.tcp_halo_phases(h) == 5
-    plane = 16 * 12 * 8
     assert [B.tcp_halo_message_bytes(h, p) for p in range(5)] == [19 * plane] + [plane] * 4
     assert B.tcp_halo_bytes(h) == 19 * plane
     box.init_fields(_np(wl.phi), None, _np(wl.T))

@@ -13,12 +13,16 @@
 
 namespace tcp {
 
+// fp64 without the phi tile: three blocks per SM (80 registers, 20-64 B of spills) measured 1 % faster on RK4 than two
+#ifndef TCP_RK_B3
+#define TCP_RK_B3 1
+#endif
 constexpr int kRkTX = 32, kRkTY = 8, kRkCZ = 32;   // chunks of 16-100 planes: within 1 % (profiles/r01_notes.md section 8)
 // Residency (profiles/r01_notes.md section 8): with the cell data requested one plane ahead the fp64 kernel needs
 // 119 registers -> 2 blocks of 256 per SM without spills (3 blocks: 80-116 B of spills and 8-15 % slower);
 // the fp32 kernel fits 3 blocks.
-template <typename real>
-constexpr int rk_min_blocks() { return sizeof(real) == 8 ? 2 : 3; }
+template <typename real, bool HAS_DK>
+constexpr int rk_min_blocks() { return sizeof(real) == 8 && (HAS_DK || !TCP_RK_B3) ? 2 : 3; }
 
 template <typename real>
 struct Plane3 {          // in-plane reductions of one field on one z plane
@@ -31,7 +35,7 @@ struct Plane3 {          // in-plane reductions of one field on one z plane
 // HAS_DK = (kappa_H != kappa_L): with equal conductivities grad kappa . grad T of eq. 4 vanishes identically, so the
 // phi tile, its nine shared loads and its reductions are left out and phi is read at the cell only (for rho c_p).
 template <typename real, bool WALLS, int MODE, bool HAS_Q, bool HAS_DK>
-__global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real>()) rk_stage_march_kernel(const RkArgs<real> R) {
+__global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real, HAS_DK>()) rk_stage_march_kernel(const RkArgs<real> R) {
     const StepArgs<real>& A = R.S;
     constexpr int TX = kRkTX, TY = kRkTY, PX = TX + 2, PY = TY + 2, PE = PX * PY;
     __shared__ real tileY[2][PE], tileP[2][PE];

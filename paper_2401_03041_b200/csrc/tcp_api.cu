@@ -186,16 +186,27 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
 
 unsigned grid_for(size_t n) { return (unsigned)((n + tcp::kBlock - 1) / tcp::kBlock); }
 
-// the z-marching stage kernel is instantiated per (walls, RkArgs::mode, heat source present)
+// the z-marching stage kernel is instantiated per (walls, RkArgs::mode, heat source present, kappa_H != kappa_L)
+template <typename real, bool WALLS, int MODE, bool HAS_Q, bool HAS_DK>
+void launch_rk_march_inst(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
+    auto kern = tcp::rk_stage_march_kernel<real, WALLS, MODE, HAS_Q, HAS_DK>;
+    const size_t ring_bytes = tcp::rk_ring_bytes<real>();        // cell-data ring (dynamic shared memory)
+    static bool configured = false;                              // once per instantiation: static + dynamic can exceed 48 KB
+    if (!configured) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ring_bytes);
+        configured = true;
+    }
+    kern<<<grid, block, ring_bytes, s->stream>>>(R);
+}
 template <typename real, bool WALLS, int MODE>
 void launch_rk_march_q(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
     const bool dk = s->P.kappa_H != s->P.kappa_L;       // grad kappa . grad T present
     if (R.S.q_src) {
-        if (dk) tcp::rk_stage_march_kernel<real, WALLS, MODE, true, true><<<grid, block, 0, s->stream>>>(R);
-        else tcp::rk_stage_march_kernel<real, WALLS, MODE, true, false><<<grid, block, 0, s->stream>>>(R);
+        if (dk) launch_rk_march_inst<real, WALLS, MODE, true, true>(s, R, grid, block);
+        else launch_rk_march_inst<real, WALLS, MODE, true, false>(s, R, grid, block);
     } else {
-        if (dk) tcp::rk_stage_march_kernel<real, WALLS, MODE, false, true><<<grid, block, 0, s->stream>>>(R);
-        else tcp::rk_stage_march_kernel<real, WALLS, MODE, false, false><<<grid, block, 0, s->stream>>>(R);
+        if (dk) launch_rk_march_inst<real, WALLS, MODE, false, true>(s, R, grid, block);
+        else launch_rk_march_inst<real, WALLS, MODE, false, false>(s, R, grid, block);
     }
 }
 template <typename real, bool WALLS>

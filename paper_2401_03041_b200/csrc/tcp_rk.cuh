@@ -14,6 +14,9 @@
 namespace tcp {
 
 // fp64 without the phi tile: three blocks per SM (80 registers, 20-64 B of spills) measured 1 % faster on RK4 than two
+#ifndef TCP_RK_RING
+#define TCP_RK_RING 3
+#endif
 #ifndef TCP_RK_B3
 #define TCP_RK_B3 1
 #endif
@@ -23,6 +26,10 @@ constexpr int kRkTX = 32, kRkTY = 8, kRkCZ = 32;   // chunks of 16-100 planes: w
 // the fp32 kernel fits 3 blocks.
 template <typename real, bool HAS_DK>
 constexpr int rk_min_blocks() { return sizeof(real) == 8 && (HAS_DK || !TCP_RK_B3) ? 2 : 3; }
+
+// bytes of the cell-data ring of rk_stage_march_kernel (dynamic shared memory): TCP_RK_RING planes x 7 values x the tile
+template <typename real>
+constexpr size_t rk_ring_bytes() { return (size_t)TCP_RK_RING * 7 * kRkTX * kRkTY * sizeof(real); }
 
 template <typename real>
 struct Plane3 {          // in-plane reductions of one field on one z plane
@@ -120,26 +127,45 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real, HAS_DK>()) 
     Ym = reduce_plane(tileY[0]); Yc = reduce_plane(tileY[1]);
     if (HAS_DK) { Pm = reduce_plane(tileP[0]); Pc = reduce_plane(tileP[1]); }
     __syncthreads();                       // buffer 0 may now be overwritten
-    // cell data (u, T^n, accumulator, source) of plane z0 + k are requested one iteration ahead as well
-    real nu[3] = {real(0), real(0), real(0)}, nTn = real(0), nacc = real(0), nq = real(0), nphi = real(0);
-    auto fetch_cell = [&](int zz) {
-        if (!inside) return;
-        const int c = x + sy * y + sz * zz;
-        nu[0] = A.u[c]; nu[1] = A.u[N + c]; nu[2] = A.u[2 * N + c];
-        if (MODE != 3) nTn = R.Tn[c];             // the last RK4 stage adds to the accumulator only
-        if (MODE >= 2) nacc = R.acc_in[c];
-        if (HAS_Q) nq = A.q_src[c];
-        if (!HAS_DK) nphi = A.phi_in[c];
+    // cell data (u, T^n, accumulator, source, phi) of plane z0 + k: every thread copies its own cell's values D - 1 planes
+    // ahead (RK4 -1.5 % against one plane ahead in registers, profiles/r01_notes.md section 23) with cp.async into its slot of a shared-memory ring (it reads only what it copied itself, so
+    // cp.async.wait_group is all the synchronisation this needs); no registers are held while they are in flight
+    constexpr int D = TCP_RK_RING, NV = 7, RING = NV * TX * TY;
+    extern __shared__ __align__(16) unsigned char rk_ring_raw[];
+    real* ring = reinterpret_cast<real*>(rk_ring_raw);
+    auto request_cell = [&](int k) {          // plane z0 + k -> ring slot k % D
+        if (inside && k < nzc) {
+            const int c = x + sy * y + sz * (z0 + k);
+            real* slot = ring + (k % D) * RING + tid;
+            cp_async_elem<real>(slot, A.u + c);
+            cp_async_elem<real>(slot + TX * TY, A.u + N + c);
+            cp_async_elem<real>(slot + 2 * TX * TY, A.u + 2 * N + c);
+            if (MODE != 3) cp_async_elem<real>(slot + 3 * TX * TY, R.Tn + c);
+            if (MODE >= 2) cp_async_elem<real>(slot + 4 * TX * TY, R.acc_in + c);
+            if (HAS_Q) cp_async_elem<real>(slot + 5 * TX * TY, A.q_src + c);
+            if (!HAS_DK) cp_async_elem<real>(slot + 6 * TX * TY, A.phi_in + c);
+        }
+        cp_async_commit();                    // one group per plane, empty or not: the wait below counts groups
     };
-    fetch_cell(z0);
+#pragma unroll
+    for (int j = 0; j < D - 1; ++j) request_cell(j);
     const real c_out = R.c_out, c_acc = R.c_acc;
     // one plane: (Ym, Yc) and (Pm, Pc) hold planes z-1, z; Yp / Pp receive plane z+1
     auto plane = [&](int k, const Plane3<real>& Ym, const Plane3<real>& Yc, Plane3<real>& Yp,
                      const Plane3<real>& Pm, const Plane3<real>& Pc, Plane3<real>& Pp) {
         const int buf = k & 1;
         const int cell = x + sy * y + sz * (z0 + k);
-        const real u[3] = {nu[0], nu[1], nu[2]}, Tn = nTn, acc = nacc, qT = nq, phi_here = nphi;
-        if (k + 1 < nzc) fetch_cell(z0 + k + 1);
+        request_cell(k + D - 1);
+        cp_async_wait<D - 1>();                    // plane k's group has landed
+        const real* slot = ring + (k % D) * RING + tid;
+        real u[3] = {real(0), real(0), real(0)}, Tn = real(0), acc = real(0), qT = real(0), phi_here = real(0);
+        if (inside) {
+            u[0] = slot[0]; u[1] = slot[TX * TY]; u[2] = slot[2 * TX * TY];
+            if (MODE != 3) Tn = slot[3 * TX * TY];
+            if (MODE >= 2) acc = slot[4 * TX * TY];
+            if (HAS_Q) qT = slot[5 * TX * TY];
+            if (!HAS_DK) phi_here = slot[6 * TX * TY];
+        }
         store_plane(buf);                          // plane z0 + k + 1
         if (k + 1 < nzc) fetch_plane(z0 + k + 2);  // next one: its latency hides behind this iteration
         __syncthreads();

@@ -10,7 +10,7 @@ namespace {
 
 template <typename real, int QT, bool WALLS, int MODE, int AA>
 cudaError_t launch_staged(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
-    const size_t smem = (size_t)(54 + QT) * kBlock * sizeof(real);
+    const size_t smem = (size_t)(54 + QT - (h_direct<real, QT, AA>() ? 27 : 0)) * kBlock * sizeof(real);
     auto kern = fused_step_async_kernel<real, QT, WALLS, MODE, AA>;
     static bool configured = false;      // once per instantiation (one device per process): saves ~1 us per launch
     if (!configured) {

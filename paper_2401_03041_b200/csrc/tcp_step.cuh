@@ -405,14 +405,26 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
 // D3Q15 / D3Q19 variants would take 212-224 KB of the SM's 256 KB, leaving almost no L1 for the
 // phi / T stencil loads (measured 0.65 of the HBM peak against 0.81-0.84 for D3Q7 and for D3Q27, which
 // only fits two blocks anyway), so those are compiled for two blocks per SM.
-template <typename real, int QT>
+// fp64 D3Q15 / D3Q19: h, which is consumed first, is pulled straight into registers together with the stencil loads and
+// only g and f are staged (42 / 46 KB per block), so that three blocks fit the shared memory as for D3Q7: 400^3 D3Q15
+// 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained; D3Q27 (15.16 -> 15.30) and D3Q7 (which has its three blocks
+// anyway) do not gain and keep h staged (profiles/r01_notes.md sections 13, 26)
+#ifndef TCP_HDIRECT
+#define TCP_HDIRECT 1
+#endif
+// (two-grid streaming only: with AA in place the same change costs 8-16 %)
+template <typename real, int QT, int AA>
+__host__ __device__ constexpr bool h_direct() { return TCP_HDIRECT && sizeof(real) == 8 && (QT == 15 || QT == 19) && AA == 0; }
+
+template <typename real, int QT, int AA = 0>
 __host__ __device__ constexpr int async_min_blocks() {
     if (sizeof(real) == 4) return 5;   // fp32: 31 KB of staging per block, <= 102 registers; 5 blocks measured +2.7 % over 4
+    if (h_direct<real, QT, AA>()) return TCP_MINB;
     return (sizeof(real) == 8 && QT >= 15) ? 2 : TCP_MINB;
 }
 
 template <typename real, int QT, bool WALLS, int MODE, int AA>
-__global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_step_async_kernel(const StepArgs<real> A) {
+__global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT, AA>()) fused_step_async_kernel(const StepArgs<real> A) {
     extern __shared__ __align__(16) unsigned char smem_raw_async[];
     real* stage = reinterpret_cast<real*>(smem_raw_async);     // [54 + QT][kBlock]
     const int tid = threadIdx.x;
@@ -451,16 +463,24 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
     };
 
     real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
+    constexpr bool HD = h_direct<real, QT, AA>();
+    constexpr int SO = HD ? -27 : 0;                              // slot offset of g and f when h is not staged
+    real hd[HD ? 27 : 1];
+    if constexpr (HD) {
 #pragma unroll
-    for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + q * kBlock + tid, src_of(A.h_in, 27, q, q));
+        for (int q = 0; q < 27; ++q) hd[q] = *src_of(A.h_in, 27, q, q);
+    } else {
+#pragma unroll
+        for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + q * kBlock + tid, src_of(A.h_in, 27, q, q));
+    }
     cp_async_commit();
 #pragma unroll
-    for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + (27 + q) * kBlock + tid, src_of(A.g_in, 27, q, q));
+    for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + (SO + 27 + q) * kBlock + tid, src_of(A.g_in, 27, q, q));
     cp_async_commit();
     if constexpr (QT > 0) {
         static_for<0, QT>([&](auto K) {
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
-            cp_async_elem<real>(stage + (54 + k) * kBlock + tid, src_of(A.f_in, QT, k, q));
+            cp_async_elem<real>(stage + (SO + 54 + k) * kBlock + tid, src_of(A.f_in, QT, k, q));
         });
     }
     cp_async_commit();
@@ -477,14 +497,14 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
     real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
 
     // (not in the calibration kernel: without arithmetic its blocks are too short-lived, measured 10.98 ms with against 10.5 ms without)
-    if constexpr (MODE != 3) prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT>());
+    if constexpr (MODE != 3) prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT, AA>());
 
     real phi_new;
     {
         cp_async_wait<2>();
         real h[27];
 #pragma unroll
-        for (int q = 0; q < 27; ++q) h[q] = stage[q * kBlock + tid];
+        for (int q = 0; q < 27; ++q) h[q] = HD ? hd[HD ? q : 0] : stage[q * kBlock + tid];
         if constexpr (MODE == 3) phi_new = phi_c; else phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
         if (active) {
 #pragma unroll
@@ -496,7 +516,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
         cp_async_wait<1>();
         real g[27];
 #pragma unroll
-        for (int q = 0; q < 27; ++q) g[q] = stage[(27 + q) * kBlock + tid];
+        for (int q = 0; q < 27; ++q) g[q] = stage[(SO + 27 + q) * kBlock + tid];
         if (WALLS && aa != 1 && A.moving) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) g[q] += wall_velocity_term<real, WALLS>(A, nb, q);
@@ -527,7 +547,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT>()) fused_st
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
             int face = 0;
             const int ax = aa == 1 ? -1 : nb.crossed(-cx27(q), -cy27(q), -cz27(q), face);
-            const real v = stage[(54 + k) * kBlock + tid];
+            const real v = stage[(SO + 54 + k) * kBlock + tid];
             if (WALLS && ax >= 0)   // anti-bounce-back (S9): the staged value is f~_opp of the own cell
                 f[k] = real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, -cx27(q), -cy27(q), -cz27(q)) - v;
             else

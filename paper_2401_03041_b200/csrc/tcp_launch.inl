@@ -83,7 +83,7 @@ cudaError_t thermal_by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaS
 // packed-pair single-precision kernels (tcp_pair.cuh)
 template <int QT, bool WALLS, int MODE, int AA>
 cudaError_t launch_pair(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_t stream) {
-    const size_t smem = (size_t)(54 + QT) * kBlock * sizeof(float2);
+    const size_t smem = (size_t)(54 + QT - (pair_h_direct<QT, AA>() ? 27 : 0)) * kBlock * sizeof(float2);
     auto kern = fused_step_pair_kernel<QT, WALLS, MODE, AA>;
     static bool configured = false;
     if (!configured) {

@@ -125,11 +125,19 @@ __device__ __forceinline__ void stencil27_pair(const StepArgs<f32x2>& A, const N
     lap = f32x2(6.0) * (((SS[0] + SS[2]) * c16 + SS[1] * c23) - centre);
 }
 
-template <int QT>
-__host__ __device__ constexpr int pair_min_blocks() { return QT >= 15 ? 2 : TCP_MINB; }   // same staging footprint as the fp64 kernels
+// Q_T >= 15, two-grid: h is pulled straight into registers and only g and f are staged, so that three blocks fit the
+// shared memory (as in the fp64 D3Q15 / D3Q19 kernels, tcp_step.cuh): 512^3 D3Q15 16.70 -> 16.03 ms, D3Q19 17.29 -> 16.42,
+// D3Q27 18.55 -> 18.35 sustained (profiles/r01_notes.md section 26)
+#ifndef TCP_PAIR_HDIRECT
+#define TCP_PAIR_HDIRECT 1
+#endif
+template <int QT, int AA>
+__host__ __device__ constexpr bool pair_h_direct() { return TCP_PAIR_HDIRECT && QT >= 15 && AA == 0; }
+template <int QT, int AA = 0>
+__host__ __device__ constexpr int pair_min_blocks() { return (QT >= 15 && !pair_h_direct<QT, AA>()) ? 2 : TCP_MINB; }
 
 template <int QT, bool WALLS, int MODE, int AA>
-__global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair_kernel(const StepArgs<f32x2> A) {
+__global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_pair_kernel(const StepArgs<f32x2> A) {
     using real = f32x2;
     extern __shared__ __align__(16) unsigned char smem_raw_pair[];
     float2* stage = reinterpret_cast<float2*>(smem_raw_pair) + threadIdx.x;     // [54 + QT][kBlock], this thread's column
@@ -171,14 +179,34 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair
         else { r[nb.first(cx)] = v.v.x; r[nb.second(cx)] = v.v.y; }
     };
 
+    // the same addressing with plain loads (pair_h_direct)
+    auto fetch = [&](const float* base, int Q, int k, int q27i) -> float2 {
+        const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
+        if (aa == 1) return *reinterpret_cast<const float2*>(base + k * N + cell);
+        int face = 0;
+        const bool bb = WALLS && nb.crossed(-cy, -cz, face) >= 0;
+        const int plane = (bb != (aa == 2)) ? Q - 1 - k : k;
+        if (bb) return *reinterpret_cast<const float2*>(base + plane * N + cell);
+        const float* r = base + plane * N + nb.row(-cy, -cz);
+        if (cx == 0) return *reinterpret_cast<const float2*>(r);
+        return make_float2(r[nb.first(-cx)], r[nb.second(-cx)]);
+    };
+    constexpr bool HD = pair_h_direct<QT, AA>();
+    constexpr int SO = HD ? -27 : 0;
+    float2 hd[HD ? 27 : 1];
+    if constexpr (HD) {
 #pragma unroll
-    for (int q = 0; q < 27; ++q) issue(stage + q * kBlock, A.h_in, 27, q, q);
+        for (int q = 0; q < 27; ++q) hd[q] = fetch(A.h_in, 27, q, q);
+    } else {
+#pragma unroll
+        for (int q = 0; q < 27; ++q) issue(stage + q * kBlock, A.h_in, 27, q, q);
+    }
     cp_async_commit();
 #pragma unroll
-    for (int q = 0; q < 27; ++q) issue(stage + (27 + q) * kBlock, A.g_in, 27, q, q);
+    for (int q = 0; q < 27; ++q) issue(stage + (SO + 27 + q) * kBlock, A.g_in, 27, q, q);
     cp_async_commit();
     if constexpr (QT > 0)
-        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; issue(stage + (54 + k) * kBlock, A.f_in, QT, k, q_of(QT, k)); });
+        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; issue(stage + (SO + 54 + k) * kBlock, A.f_in, QT, k, q_of(QT, k)); });
     cp_async_commit();
 
     real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
@@ -188,14 +216,14 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair
 #pragma unroll
     for (int al = 0; al < 3; ++al) { const float2 t = *reinterpret_cast<const float2*>(A.u + al * N + cell); u[al] = real(t.x, t.y); }
 
-    prefetch_next_wave<float, QT, AA, StepArgs<f32x2>>(A, 2 * kBlock, pair_min_blocks<QT>());
+    prefetch_next_wave<float, QT, AA, StepArgs<f32x2>>(A, 2 * kBlock, pair_min_blocks<QT, AA>());
 
     real phi_new;
     {
         cp_async_wait<2>();
         real h[27];
 #pragma unroll
-        for (int q = 0; q < 27; ++q) h[q].v = stage[q * kBlock];
+        for (int q = 0; q < 27; ++q) h[q].v = HD ? hd[HD ? q : 0] : stage[q * kBlock];
         phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
         if (active) {
 #pragma unroll
@@ -207,7 +235,7 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair
         cp_async_wait<1>();
         real g[27];
 #pragma unroll
-        for (int q = 0; q < 27; ++q) g[q].v = stage[(27 + q) * kBlock];
+        for (int q = 0; q < 27; ++q) g[q].v = stage[(SO + 27 + q) * kBlock];
         if (WALLS && aa != 1 && A.moving) {
 #pragma unroll
             for (int q = 0; q < 27; ++q) g[q] += wall_velocity_term_pair(A, nb, q);
@@ -242,7 +270,7 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT>()) fused_step_pair
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
             int face = 0;
             const int ax = aa == 1 ? -1 : nb.crossed(-cy27(q), -cz27(q), face);
-            real v; v.v = stage[(54 + k) * kBlock];
+            real v; v.v = stage[(SO + 54 + k) * kBlock];
             if (WALLS && ax >= 0)   // anti-bounce-back (S9): T_w at the tangential position of each lane's source cell
                 v = real(2.0 * weight(QT, cls27(q))) * wall_temperature_pair(A, nb, ax, face, -cx27(q), -cy27(q), -cz27(q)) - v;
             f[k] = v;

@@ -125,14 +125,15 @@ __device__ __forceinline__ void stencil27_pair(const StepArgs<f32x2>& A, const N
     lap = f32x2(6.0) * (((SS[0] + SS[2]) * c16 + SS[1] * c23) - centre);
 }
 
-// Q_T >= 15, two-grid: h is pulled straight into registers and only g and f are staged, so that three blocks fit the
-// shared memory (as in the fp64 D3Q15 / D3Q19 kernels, tcp_step.cuh): 512^3 D3Q15 16.70 -> 16.03 ms, D3Q19 17.29 -> 16.42,
-// D3Q27 18.55 -> 18.35 sustained (profiles/r01_notes.md section 26)
+// Thermal LB, two-grid: h is pulled straight into registers and only g and f are staged; for Q_T >= 15 three blocks then fit
+// the shared memory (as in the fp64 D3Q15 / D3Q19 kernels, tcp_step.cuh): 512^3 D3Q15 16.70 -> 16.03 ms, D3Q19 17.29 -> 16.42,
+// D3Q27 18.55 -> 18.35, D3Q7 (three blocks either way) 14.34 -> 14.02 sustained; the RK paths (Q_T = 0) lose 0.5-1 % and keep h
+// staged (profiles/r01_notes.md section 26)
 #ifndef TCP_PAIR_HDIRECT
 #define TCP_PAIR_HDIRECT 1
 #endif
 template <int QT, int AA>
-__host__ __device__ constexpr bool pair_h_direct() { return TCP_PAIR_HDIRECT && QT >= 15 && AA == 0; }
+__host__ __device__ constexpr bool pair_h_direct() { return TCP_PAIR_HDIRECT && QT > 0 && AA == 0; }
 template <int QT, int AA = 0>
 __host__ __device__ constexpr int pair_min_blocks() { return (QT >= 15 && !pair_h_direct<QT, AA>()) ? 2 : TCP_MINB; }
 

@@ -407,8 +407,9 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
 // only fits two blocks anyway), so those are compiled for two blocks per SM.
 // fp64 D3Q15 / D3Q19: h, which is consumed first, is pulled straight into registers together with the stencil loads and
 // only g and f are staged (42 / 46 KB per block), so that three blocks fit the shared memory as for D3Q7: 400^3 D3Q15
-// 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained; D3Q27 (15.16 -> 15.30) and D3Q7 (which has its three blocks
-// anyway) do not gain and keep h staged (profiles/r01_notes.md sections 13, 26)
+// 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained.  D3Q27 (15.16 -> 15.30) keeps h staged, and so does D3Q7, which
+// has its three blocks anyway: 0.5 % faster under the power cap but 4 % slower per launch at full clock (ncu 10.79 vs
+// 10.35 ms, 2 % more DRAM reads) (profiles/r01_notes.md sections 13, 26)
 #ifndef TCP_HDIRECT
 #define TCP_HDIRECT 1
 #endif

@@ -59,6 +59,11 @@ typedef struct tcpo_params {
     double wall_u[3][2][3];            /* wall velocity per axis / face (moving wall; reading S18) */
     double sigma_TT;                   /* d^2 sigma / dT^2: "parabolic (or non-linear) relation between surface tension and
                                           temperature" (reading S19); 0 = the linear eq. 9 */
+    /* ---- oracle-only switches (no counterpart in the CUDA library) ---- */
+    int hydro_phi_level;               /* which phi the hydrodynamic update differentiates: 0 = phi^n (reading S16, what
+                                          Algorithm 1's communication order implies), 1 = phi^{n+1}
+                                          (SURVEY O5's proposal).  Exists so that tests/test_oracle_s16.py can show what
+                                          the alternative does on the paper's own channel benchmark */
 } tcpo_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -716,8 +721,9 @@ int tcpo_step(tcpo_sim *s, int nsteps) {
     for (int n = 0; n < nsteps; n++) {
         int rc;
         if ((rc = update_h(s))) return rc;
+        if (s->P.hydro_phi_level == 1) { double *t = s->phi; s->phi = s->phi2; s->phi2 = t; } /* O5 as SURVEY proposed it */
         if ((rc = update_g(s))) return rc;
-        { double *t = s->phi; s->phi = s->phi2; s->phi2 = t; } /* phi^{n+1} becomes current (S16) */
+        if (s->P.hydro_phi_level != 1) { double *t = s->phi; s->phi = s->phi2; s->phi2 = t; } /* phi^{n+1} becomes current (S16) */
         if ((rc = s->thermal_is_lb ? update_f(s) : update_T_rk(s))) return rc;
         s->steps_done++;
     }

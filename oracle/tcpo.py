@@ -32,6 +32,7 @@ class Params(C.Structure):
         ("eps_normal", C.c_double),
         ("wall_u", ((C.c_double * 3) * 2) * 3),
         ("sigma_TT", C.c_double),
+        ("hydro_phi_level", C.c_int),      # oracle-only (reading S16): 0 = phi^n, 1 = phi^{n+1}
     ]
 
 
@@ -44,6 +45,7 @@ DEFAULTS = dict(
     s_bulk=1.0, s_high=1.0, high_rate_equals_shear=0, eps_normal=1e-32,
     wall_u=(((0.0,) * 3,) * 2,) * 3,
     sigma_TT=0.0,
+    hydro_phi_level=0,
 )
 
 
@@ -69,6 +71,7 @@ def make_params(d: dict) -> Params:
               "kappa_H", "kappa_L", "cp_H", "cp_L", "s_bulk", "s_high", "eps_normal"):
         setattr(p, k, float(v[k]))
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
+    p.hydro_phi_level = int(v["hydro_phi_level"])
     for a in range(3):
         for f in range(2):
             for c in range(3):

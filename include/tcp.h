@@ -66,18 +66,28 @@ typedef struct tcp_params {
                                           Default 0 = eq. 9 as printed */
 } tcp_params;
 
+/* Fill *p with the defaults: struct_size, fp64, thermal LB D3Q7, two-grid, periodic x 3, rho = 1, tau = 0.6, xi = 4,
+ * M = 0.05, sigma = 0, kappa = 0.2, c_p = 1, no gravity, walls at rest and at T = 0, s_bulk = s_high = 1 (the closed-form
+ * central-moment collision), eps_normal = 1e-32.  A zero-initialised struct is NOT valid (eps_normal = 0 makes the
+ * interface normal 0/0 in the bulk, s_bulk = s_high = 0 are not relaxation rates): tcp_create rejects it with TCP_EINVAL.
+ * Errors: TCP_EINVAL (p NULL). */
+int tcp_params_default(tcp_params *p);
+
 /* Bytes of device memory one simulation needs (populations, fields, wall planes).
  * Errors: TCP_EINVAL (bad extents / parameters), TCP_EUNSUPPORTED. */
 int tcp_workspace_bytes(int nx, int ny, int nz, const tcp_params *p, size_t *bytes);
 
 /* Create a simulation; the library allocates the workspace (cudaMalloc) and a stream.
- * Validation: n >= 1 (>= 2 on WALLS axes), tau > -1/2, M, xi, rho, kappa, cp > 0.
+ * Validation: n >= 1 (>= 2 on WALLS axes), tau > -1/2, M, xi, rho, kappa, cp, eps_normal > 0, 0 < s_bulk, s_high < 2.
+ * The simulation lives on the CUDA device that is current at the call; every later call makes that device current
+ * for its own duration, so simulations on several GPUs can be driven from one thread.
  * Errors: TCP_EINVAL, TCP_EUNSUPPORTED, TCP_ENOMEM, TCP_ECUDA. */
 int tcp_create(int nx, int ny, int nz, const tcp_params *p, tcp_sim **out);
 
 /* Same, on caller-owned device memory (>= tcp_workspace_bytes, 256-byte aligned) and on the
  * caller's CUDA stream (a cudaStream_t passed as void*; NULL = default stream).  The memory and
- * the stream must outlive the simulation. */
+ * the stream must outlive the simulation.  The simulation lives on the device that owns the workspace (resolved with
+ * cudaPointerGetAttributes); the stream must belong to the same device. */
 int tcp_create_in(int nx, int ny, int nz, const tcp_params *p, void *dev_workspace, size_t bytes,
                   void *cuda_stream, tcp_sim **out);
 
@@ -86,7 +96,9 @@ int tcp_create_in(int nx, int ny, int nz, const tcp_params *p, void *dev_workspa
  * u == NULL -> 0; T == NULL -> T_ref.  Errors: TCP_EINVAL (phi NULL), TCP_ECUDA. */
 int tcp_init_fields(tcp_sim *s, const void *phi, const void *u, const void *T);
 
-/* Per-wall-cell Dirichlet temperature (eq. 30); Tw == NULL restores the constant wall_T. */
+/* Per-wall-cell Dirichlet temperature (eq. 30); Tw == NULL restores the constant wall_T.  May be called at any time
+ * between steps; the new plane acts from the next step on, identically for both streaming patterns (with TCP_STREAM_AA
+ * the wall links that are stored already anti-bounced are corrected for the change). */
 int tcp_set_wall_temperature(tcp_sim *s, int axis, int face, const void *Tw);
 
 /* Volumetric heat source q_T [nz][ny][nx] of eqs. 4 / 27 (e.g. eq. 37); NULL (default) = none. */
@@ -163,6 +175,8 @@ int tcp_last_step_ms(tcp_sim *s, float *ms);
  * access pattern and staging of the fused step (same pulls, same stores) but no stencils and no collision,
  * and return its mean duration.  It reads the current state and overwrites only the spare grid and the
  * spare phi / T buffers, so the simulation is unchanged -- except u, which is rewritten with itself.
+ * It times itself with events of its own and is not counted by tcp_launch_count, so tcp_last_step_ms and
+ * tcp_launch_count keep describing the method's kernels only.
  * Errors: TCP_ESTATE, TCP_EINVAL, TCP_EUNSUPPORTED (walls or AA streaming). */
 int tcp_pattern_copy_ms(tcp_sim *s, int nlaunches, float *ms);
 

@@ -3,7 +3,7 @@
 The product is the C-ABI CUDA library `libtcp.so` (include/tcp.h, csrc/); this package is its thin
 Python binding.  See DESIGN.md.
 """
-from .binding import (Simulation, TcpError, make_params, tcp_params, lib, library_path, EXPORTS,
+from .binding import (Simulation, TcpError, make_params, tcp_params, lib, library_path, EXPORTS, tcp_params_default,
                       tcp_workspace_bytes, tcp_create, tcp_create_in, tcp_init_fields,
                       tcp_set_wall_temperature, tcp_set_heat_source, tcp_step, tcp_relax_temperature, tcp_read_fields,
                       tcp_synchronize, tcp_launch_count, tcp_last_step_ms, tcp_pattern_copy_ms, tcp_destroy, tcp_last_error,

@@ -80,7 +80,7 @@ def make_params(d: dict) -> tcp_params:
     return p
 
 
-EXPORTS = ["tcp_workspace_bytes", "tcp_create", "tcp_create_in", "tcp_init_fields", "tcp_set_wall_temperature",
+EXPORTS = ["tcp_params_default", "tcp_workspace_bytes", "tcp_create", "tcp_create_in", "tcp_init_fields", "tcp_set_wall_temperature",
            "tcp_set_heat_source", "tcp_step", "tcp_relax_temperature", "tcp_read_fields", "tcp_synchronize", "tcp_launch_count",
            "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_destroy", "tcp_last_error",
            "tcp_set_halo", "tcp_halo_phases", "tcp_halo_message_bytes", "tcp_halo_bytes", "tcp_step_begin", "tcp_step_advance",
@@ -100,6 +100,7 @@ def lib():
         path = _build.build()
         L = C.CDLL(path)
         vp, pp = C.c_void_p, C.POINTER(tcp_params)
+        L.tcp_params_default.argtypes = [pp]
         L.tcp_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, pp, C.POINTER(C.c_size_t)]
         L.tcp_create.argtypes = [C.c_int, C.c_int, C.c_int, pp, C.POINTER(vp)]
         L.tcp_create_in.argtypes = [C.c_int, C.c_int, C.c_int, pp, vp, C.c_size_t, vp, C.POINTER(vp)]
@@ -150,6 +151,12 @@ def _ptr(a):
 
 
 # ---- the ABI, name for name -------------------------------------------------------------------
+
+def tcp_params_default() -> tcp_params:
+    p = tcp_params()
+    _check(lib().tcp_params_default(C.byref(p)))
+    return p
+
 
 def tcp_workspace_bytes(nx, ny, nz, params: tcp_params) -> int:
     n = C.c_size_t()

@@ -8,7 +8,6 @@
 #include <new>
 
 #include "../../include/tcp.h"
-#include <cstdlib>
 
 #include "tcp_halo.cuh"
 #include "tcp_launch.h"
@@ -68,7 +67,11 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
     if (!(p->M > 0) || !(p->xi > 0)) return fail(TCP_EINVAL, "M and xi must be > 0");
     if (!(p->rho_H > 0) || !(p->rho_L > 0)) return fail(TCP_EINVAL, "rho must be > 0");
     if (!(p->kappa_H > 0) || !(p->kappa_L > 0) || !(p->cp_H > 0) || !(p->cp_L > 0)) return fail(TCP_EINVAL, "kappa and cp must be > 0");
-    if (!(p->eps_normal >= 0)) return fail(TCP_EINVAL, "eps_normal must be >= 0");
+    // eps_normal = 0 would make n = grad phi / |grad phi| a 0/0 in every uniform bulk cell (reading S8): a caller who
+    // zero-initialises the struct gets an error, not NaNs; tcp_params_default() fills the documented defaults
+    if (!(p->eps_normal > 0)) return fail(TCP_EINVAL, "eps_normal must be > 0 (default 1e-32, see tcp_params_default)");
+    if (!(p->s_bulk > 0 && p->s_bulk < 2) || !(p->s_high > 0 && p->s_high < 2)) return fail(TCP_EINVAL, "s_bulk and s_high must lie in (0, 2) (default 1, see tcp_params_default)");
+    if (p->high_rate_equals_shear != 0 && p->high_rate_equals_shear != 1) return fail(TCP_EINVAL, "high_rate_equals_shear must be 0 or 1");
     return TCP_OK;
 }
 
@@ -112,7 +115,8 @@ struct tcp_sim {
     bool initialised, has_q, walls, stepped;
     long long launches;
     cudaEvent_t ev0, ev1;
-    bool use_async;          // cp.async staged kernel
+    cudaEvent_t evc0, evc1;  // tcp_pattern_copy_ms only: the calibration must not disturb tcp_last_step_ms
+    int device;              // the CUDA device the workspace lives on; every entry point runs with it current
     bool use_pair;           // fp32: two cells per thread, packed arithmetic (x periodic, nx even)
     int aa_next;             // AA streaming: type of the next step (1 even, 2 odd); 0 = two-grid
     // z-slab of a decomposed box (tcp_set_halo): plane 0 / nz-1 is a ghost plane filled from a neighbour
@@ -128,6 +132,17 @@ struct tcp_sim {
 namespace {
 
 template <typename real> real* ptr(const tcp_sim* s, size_t off) { return reinterpret_cast<real*>(s->base + off); }
+
+// Makes the simulation's device current for the duration of an entry point and restores the caller's afterwards,
+// so that several simulations on several GPUs can be driven from one thread.
+struct DeviceScope {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceScope(const tcp_sim* s) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != s->device) switched = cudaSetDevice(s->device) == cudaSuccess;
+    }
+    ~DeviceScope() { if (switched) cudaSetDevice(prev); }
+};
 
 // constants {m, s1, s2} of tcp::fast_div for the divisor d >= 1
 void fast_div_make(unsigned d, unsigned c[3]) {
@@ -191,12 +206,10 @@ template <typename real, bool WALLS, int MODE, bool HAS_Q, bool HAS_DK>
 void launch_rk_march_inst(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
     auto kern = tcp::rk_stage_march_kernel<real, WALLS, MODE, HAS_Q, HAS_DK>;
     const size_t ring_bytes = tcp::rk_ring_bytes<real>();        // cell-data ring (dynamic shared memory)
-    static bool configured = false;                              // once per instantiation: static + dynamic can exceed 48 KB
-    if (!configured) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ring_bytes);
-        configured = true;
-    }
-    kern<<<grid, block, ring_bytes, s->stream>>>(R);
+    static bool configured[tcp::kMaxDevices] = {};               // once per instantiation and device: static + dynamic can exceed 48 KB
+    if (!configured[s->device])
+        configured[s->device] = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ring_bytes) == cudaSuccess;
+    kern<<<grid, block, ring_bytes, s->stream>>>(R);       // a failed attribute call surfaces here as a launch error (cudaGetLastError)
 }
 template <typename real, bool WALLS, int MODE>
 void launch_rk_march_q(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, dim3 block) {
@@ -227,15 +240,9 @@ void launch_rk_march(const tcp_sim* s, const tcp::RkArgs<real>& R, dim3 grid, di
 template <typename real>
 void launch_rk_stage(const tcp_sim* s, const tcp::RkArgs<real>& R) {
     const int P = s->nx * s->ny, planes = (R.S.cell1 - R.S.cell0) / P;       // whole planes [cell0, cell1)
-    if (s->use_async) {   // default: z-marching tile kernel (tcp_rk.cuh)
-        const dim3 block(tcp::kRkTX, tcp::kRkTY);
-        const dim3 grid((s->nx + tcp::kRkTX - 1) / tcp::kRkTX, (s->ny + tcp::kRkTY - 1) / tcp::kRkTY, (planes + tcp::kRkCZ - 1) / tcp::kRkCZ);
-        launch_rk_march<real>(s, R, grid, block);
-        return;
-    }
-    const unsigned grid = grid_for((size_t)(R.S.cell1 - R.S.cell0));
-    if (s->walls) tcp::rk_stage_kernel<real, true><<<grid, tcp::kBlock, 0, s->stream>>>(R);
-    else tcp::rk_stage_kernel<real, false><<<grid, tcp::kBlock, 0, s->stream>>>(R);
+    const dim3 block(tcp::kRkTX, tcp::kRkTY);                                 // z-marching tile kernel (tcp_rk.cuh)
+    const dim3 grid((s->nx + tcp::kRkTX - 1) / tcp::kRkTX, (s->ny + tcp::kRkTY - 1) / tcp::kRkTY, (planes + tcp::kRkCZ - 1) / tcp::kRkCZ);
+    launch_rk_march<real>(s, R, grid, block);
 }
 
 // The stages of the Runge-Kutta update of T (eqs. 25-26) from T[curT] into T[1 - curT], in order;
@@ -273,14 +280,11 @@ int rk_stages(const tcp_sim* s, const tcp::StepArgs<real>& A, const real* phi, t
     return 4;
 }
 
-// Stage 1 inside the fused kernel (rk_stage1_local, tcp_step.cuh): the Runge-Kutta paths with equal conductivities,
-// whenever a staged kernel runs the step (the register-staged A/B kernel of TCP_KERNEL=flat keeps the separate stage).
+// Stage 1 inside the fused kernel (rk_stage1_local, tcp_step.cuh): the Runge-Kutta paths with equal conductivities.
 bool rk_first_stage_fused(const tcp_sim* s) {
     const int th = s->P.thermal;
     if (th != TCP_THERMAL_RK2 && th != TCP_THERMAL_RK4) return false;
-    if (s->P.kappa_H != s->P.kappa_L) return false;
-    const bool flat = !s->use_async && !s->P.high_rate_equals_shear && s->P.s_high == 1.0 && s->P.streaming == TCP_STREAM_TWO_GRID;
-    return !flat;
+    return s->P.kappa_H == s->P.kappa_L;
 }
 
 // stages [first, n) of the Runge-Kutta update
@@ -310,7 +314,7 @@ int relax_t(tcp_sim* s, int nsteps) {
         tcp::StepArgs<real> A = make_args<real>(s);
         if (qt) {
             tcp::FusedCfg c;
-            c.qt = qt; c.walls = s->walls; c.mode = s->P.high_rate_equals_shear ? 1 : 0; c.aa = aa; c.staged = true; c.grid = grid_for(s->N);
+            c.qt = qt; c.walls = s->walls; c.mode = s->P.high_rate_equals_shear ? 1 : 0; c.aa = aa; c.device = s->device; c.grid = grid_for(s->N);
             CK(s->walls ? tcp::launch_thermal_walls(c, A, s->stream) : tcp::launch_thermal_periodic(c, A, s->stream));
             s->launches++;
             if (aa) aa = 3 - aa;
@@ -329,11 +333,10 @@ int launch_fused(tcp_sim* s, const tcp::StepArgs<real>& A) {
     // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
     const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
     tcp::FusedCfg c;
-    c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next;
-    c.staged = s->use_async || mode != 0 || c.aa != 0;
+    c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next; c.device = s->device;
     c.grid = grid_for((size_t)(A.cell1 - A.cell0));
     if constexpr (sizeof(real) == 4) {
-        if (s->use_pair && c.staged && mode == 0) {
+        if (s->use_pair && mode == 0) {
             CK(s->walls ? tcp::launch_pair_walls(c, A, s->stream) : tcp::launch_pair_periodic(c, A, s->stream));
         } else {
             CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
@@ -549,12 +552,32 @@ template <typename real>
 int fill_wall(tcp_sim* s, int axis, int face, const void* Tw) {
     const size_t plane[3] = {(size_t)s->ny * s->nz, (size_t)s->nx * s->nz, (size_t)s->nx * s->ny};
     real* dst = ptr<real>(s, s->L.wallT[axis][face]);
-    if (Tw) CK(cudaMemcpyAsync(dst, Tw, plane[axis] * sizeof(real), cudaMemcpyDefault, s->stream));
+    const int qt = thermal_q(s->P.thermal);
+    // AA streaming with the populations in the pushed layout (after tcp_init_fields or an odd step): the wall links of
+    // f~ already carry the old plane, see aa_wall_repush_kernel.  The new plane is staged in the spare phi buffer.
+    const bool repush = s->P.streaming == TCP_STREAM_AA && s->initialised && s->aa_next == 1 && qt > 0 && s->P.bc[axis] == TCP_BC_WALLS;
+    real* target = repush ? ptr<real>(s, s->L.phi[1 - s->cur]) : dst;
+    if (Tw) CK(cudaMemcpyAsync(target, Tw, plane[axis] * sizeof(real), cudaMemcpyDefault, s->stream));
     else {
-        tcp::fill_kernel<real><<<(unsigned)((plane[axis] + 255) / 256), 256, 0, s->stream>>>(dst, (long long)plane[axis],
+        tcp::fill_kernel<real><<<(unsigned)((plane[axis] + 255) / 256), 256, 0, s->stream>>>(target, (long long)plane[axis],
                                                                                         (real)s->P.wall_T[axis][face]);
         s->launches++;
         CK(cudaGetLastError());
+    }
+    if (repush) {
+        const tcp::StepArgs<real> A = make_args<real>(s);
+        real* f = ptr<real>(s, s->L.f[0]);
+        const unsigned grid = grid_for(plane[axis]);
+        const int pc = (int)plane[axis];
+        switch (qt) {
+        case 7: tcp::aa_wall_repush_kernel<real, 7><<<grid, tcp::kBlock, 0, s->stream>>>(A, f, axis, face, target, dst, pc); break;
+        case 15: tcp::aa_wall_repush_kernel<real, 15><<<grid, tcp::kBlock, 0, s->stream>>>(A, f, axis, face, target, dst, pc); break;
+        case 19: tcp::aa_wall_repush_kernel<real, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A, f, axis, face, target, dst, pc); break;
+        default: tcp::aa_wall_repush_kernel<real, 27><<<grid, tcp::kBlock, 0, s->stream>>>(A, f, axis, face, target, dst, pc); break;
+        }
+        s->launches++;
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(dst, target, plane[axis] * sizeof(real), cudaMemcpyDeviceToDevice, s->stream));
     }
     CK(cudaStreamSynchronize(s->stream));
     return TCP_OK;
@@ -600,13 +623,21 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
     s->L = make_layout(nx, ny, nz, p);
     s->walls = p->bc[0] == TCP_BC_WALLS || p->bc[1] == TCP_BC_WALLS || p->bc[2] == TCP_BC_WALLS;
     s->owns_memory = own; s->owns_stream = own;
-    {   // default: the cp.async staged kernels; TCP_KERNEL=flat selects the register-staged fused kernel and the
-        // flat RK stage kernel for A/B runs (two-grid, default collision mode only; anything else stays staged)
-        const char* force = std::getenv("TCP_KERNEL");
-        s->use_async = !(force && std::strcmp(force, "flat") == 0);
-        // fp32: the packed-pair kernel wherever its layout rules hold; TCP_KERNEL=scalar keeps one cell per thread
-        s->use_pair = p->precision == TCP_F32 && p->bc[0] == TCP_BC_PERIODIC && nx % 2 == 0 && !(force && std::strcmp(force, "scalar") == 0);
+    if (own) {
+        e = cudaGetDevice(&s->device);
+        if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaGetDevice"); }
+    } else {
+        // the workspace decides the device: memory and stream of any GPU of the process may be handed in
+        if (!workspace) { delete s; return fail(TCP_EINVAL, "workspace is NULL"); }
+        cudaPointerAttributes at;
+        e = cudaPointerGetAttributes(&at, workspace);
+        if (e != cudaSuccess || at.type != cudaMemoryTypeDevice) { cudaGetLastError(); delete s; return fail(TCP_EINVAL, "workspace is not device memory"); }
+        s->device = at.device;
     }
+    if (s->device < 0 || s->device >= tcp::kMaxDevices) { delete s; return fail(TCP_EUNSUPPORTED, "device ordinal out of range"); }
+    DeviceScope scope(s);
+    // fp32: the packed-pair kernel wherever its layout rules hold (x periodic, nx even), else one cell per thread
+    s->use_pair = p->precision == TCP_F32 && p->bc[0] == TCP_BC_PERIODIC && nx % 2 == 0;
     if (own) {
         void* mem = nullptr;
         e = cudaMalloc(&mem, s->L.total);
@@ -622,6 +653,7 @@ int create_common(int nx, int ny, int nz, const tcp_params* p, void* workspace, 
         s->stream = static_cast<cudaStream_t>(stream);
     }
     if (cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess ||
+        cudaEventCreate(&s->evc0) != cudaSuccess || cudaEventCreate(&s->evc1) != cudaSuccess ||
         cudaEventCreateWithFlags(&s->ev_bnd, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&s->ev_comm, cudaEventDisableTiming) != cudaSuccess) {
         tcp_destroy(s);
@@ -642,6 +674,21 @@ extern "C" {
 
 const char* tcp_last_error(void) { return g_err; }
 
+int tcp_params_default(tcp_params* p) {
+    if (!p) return fail(TCP_EINVAL, "params is NULL");
+    std::memset(p, 0, sizeof *p);
+    p->struct_size = sizeof(tcp_params);
+    p->precision = TCP_F64; p->thermal = TCP_THERMAL_LB_D3Q7; p->streaming = TCP_STREAM_TWO_GRID;
+    p->rho_H = p->rho_L = 1.0;
+    p->tau_H = p->tau_L = 0.6;
+    p->xi = 4.0; p->M = 0.05;
+    p->kappa_H = p->kappa_L = 0.2;
+    p->cp_H = p->cp_L = 1.0;
+    p->s_bulk = p->s_high = 1.0;
+    p->eps_normal = 1e-32;
+    return TCP_OK;
+}
+
 int tcp_workspace_bytes(int nx, int ny, int nz, const tcp_params* p, size_t* bytes) {
     if (!bytes) return fail(TCP_EINVAL, "bytes is NULL");
     int rc = validate(nx, ny, nz, p);
@@ -660,10 +707,13 @@ int tcp_create_in(int nx, int ny, int nz, const tcp_params* p, void* dev_workspa
 
 int tcp_destroy(tcp_sim* s) {
     if (!s) return TCP_OK;
+    DeviceScope scope(s);
     cudaStreamSynchronize(s->stream);
     if (s->halo[0] || s->halo[1]) cudaStreamSynchronize(s->comm);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
+    if (s->evc0) cudaEventDestroy(s->evc0);
+    if (s->evc1) cudaEventDestroy(s->evc1);
     if (s->ev_bnd) cudaEventDestroy(s->ev_bnd);
     if (s->ev_comm) cudaEventDestroy(s->ev_comm);
     if (s->owns_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -676,17 +726,20 @@ int tcp_init_fields(tcp_sim* s, const void* phi, const void* u, const void* T) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
     if (!phi) return fail(TCP_EINVAL, "phi is required");
     if (s->in_step) return fail(TCP_ESTATE, "tcp_init_fields between tcp_step_begin and tcp_step_end");
+    DeviceScope scope(s);
     return s->P.precision == TCP_F64 ? init_fields_t<double>(s, phi, u, T) : init_fields_t<float>(s, phi, u, T);
 }
 
 int tcp_set_wall_temperature(tcp_sim* s, int axis, int face, const void* Tw) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
     if (axis < 0 || axis > 2 || face < 0 || face > 1) return fail(TCP_EINVAL, "axis must be 0..2 and face 0..1");
+    DeviceScope scope(s);
     return s->P.precision == TCP_F64 ? fill_wall<double>(s, axis, face, Tw) : fill_wall<float>(s, axis, face, Tw);
 }
 
 int tcp_set_heat_source(tcp_sim* s, const void* q) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    DeviceScope scope(s);
     s->has_q = q != nullptr;
     if (q) {
         const size_t es = s->P.precision == TCP_F64 ? 8 : 4;
@@ -701,6 +754,7 @@ int tcp_step(tcp_sim* s, int nsteps) {
     if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
     if (nsteps < 0) return fail(TCP_EINVAL, "nsteps must be >= 0");
     if (s->halo[0] || s->halo[1]) return fail(TCP_ESTATE, "a slab with ghost planes steps with tcp_step_begin / tcp_step_end");
+    DeviceScope scope(s);
     CK(cudaEventRecord(s->ev0, s->stream));
     for (int n = 0; n < nsteps; ++n) {
         int rc = s->P.precision == TCP_F64 ? step_once<double>(s) : step_once<float>(s);
@@ -720,17 +774,20 @@ int tcp_relax_temperature(tcp_sim* s, int nsteps) {
     if (s->halo[0] || s->halo[1]) return fail(TCP_EUNSUPPORTED, "tcp_relax_temperature: not on a slab with ghost planes");
     if (lb && s->P.streaming == TCP_STREAM_AA && (nsteps & 1))
         return fail(TCP_EINVAL, "AA streaming: the thermal populations must keep the parity of h and g, so nsteps must be even");
+    DeviceScope scope(s);
     return s->P.precision == TCP_F64 ? relax_t<double>(s, nsteps) : relax_t<float>(s, nsteps);
 }
 
 int tcp_read_fields(tcp_sim* s, void* phi, void* u, void* p, void* T) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
     if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
+    DeviceScope scope(s);
     return s->P.precision == TCP_F64 ? read_fields_t<double>(s, phi, u, p, T) : read_fields_t<float>(s, phi, u, p, T);
 }
 
 int tcp_synchronize(tcp_sim* s) {
     if (!s) return fail(TCP_EINVAL, "sim is NULL");
+    DeviceScope scope(s);
     CK(cudaStreamSynchronize(s->stream));
     CK(cudaGetLastError());
     return TCP_OK;
@@ -775,12 +832,14 @@ int tcp_step_begin(tcp_sim* s) {
     if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
     if (!s->halo[0] && !s->halo[1]) return fail(TCP_ESTATE, "tcp_step_begin: no ghost planes (tcp_set_halo); use tcp_step");
     if (s->in_step) return fail(TCP_ESTATE, "tcp_step_begin called twice without tcp_step_end");
+    DeviceScope scope(s);
     return s->P.precision == TCP_F64 ? step_begin_t<double>(s) : step_begin_t<float>(s);
 }
 
 int tcp_step_advance(tcp_sim* s, int* transfers_left) {
     if (!s || !transfers_left) return fail(TCP_EINVAL, "NULL argument");
     if (!s->in_step) return fail(TCP_ESTATE, "tcp_step_advance without tcp_step_begin");
+    DeviceScope scope(s);
     return s->P.precision == TCP_F64 ? step_advance_t<double>(s, transfers_left) : step_advance_t<float>(s, transfers_left);
 }
 
@@ -798,19 +857,20 @@ int tcp_pattern_copy_ms(tcp_sim* s, int nlaunches, float* ms) {
     if (nlaunches < 1) return fail(TCP_EINVAL, "nlaunches must be >= 1");
     if (s->walls || s->P.streaming != TCP_STREAM_TWO_GRID || s->halo[0] || s->halo[1])
         return fail(TCP_EUNSUPPORTED, "pattern copy: periodic two-grid simulations without ghost planes only");
+    DeviceScope scope(s);
     tcp::FusedCfg c;
-    c.qt = thermal_q(s->P.thermal); c.walls = false; c.mode = 3; c.aa = 0; c.staged = true; c.grid = grid_for(s->N);
-    CK(cudaEventRecord(s->ev0, s->stream));
+    c.qt = thermal_q(s->P.thermal); c.walls = false; c.mode = 3; c.aa = 0; c.device = s->device; c.grid = grid_for(s->N);
+    // its own events, and not counted by tcp_launch_count: the calibration is not part of the method
+    CK(cudaEventRecord(s->evc0, s->stream));
     for (int i = 0; i < nlaunches; ++i) {
         // in -> out only: the simulation's current state (grid `cur`) is read, the spare grid is overwritten
         if (s->P.precision == TCP_F64) CK(tcp::launch_fused_periodic(c, make_args<double>(s), s->stream));
         else CK(tcp::launch_fused_periodic(c, make_args<float>(s), s->stream));
-        s->launches++;
     }
-    CK(cudaEventRecord(s->ev1, s->stream));
-    CK(cudaEventSynchronize(s->ev1));
+    CK(cudaEventRecord(s->evc1, s->stream));
+    CK(cudaEventSynchronize(s->evc1));
     float total = 0.f;
-    CK(cudaEventElapsedTime(&total, s->ev0, s->ev1));
+    CK(cudaEventElapsedTime(&total, s->evc0, s->evc1));
     *ms = total / nlaunches;
     return TCP_OK;
 }
@@ -818,6 +878,7 @@ int tcp_pattern_copy_ms(tcp_sim* s, int nlaunches, float* ms) {
 int tcp_last_step_ms(tcp_sim* s, float* ms) {
     if (!s || !ms) return fail(TCP_EINVAL, "NULL argument");
     if (!s->stepped) return fail(TCP_ESTATE, "tcp_step has not been called");
+    DeviceScope scope(s);
     CK(cudaEventSynchronize(s->ev1));
     CK(cudaEventElapsedTime(ms, s->ev0, s->ev1));
     return TCP_OK;

@@ -184,10 +184,13 @@ __device__ __forceinline__ real wall_velocity_term(const StepArgs<real>& A, cons
 //   grad_x = D_x S_y S_z,  lap = 6 (S_x S_y S_z - 1),   S = [1/6, 2/3, 1/6],  D = [-1/2, 0, 1/2]
 // IS_TEMP: Dirichlet ghost 2 T_w - T(mirror); otherwise ghost = mirror cell (phi, neutral wetting).
 
+// The 1/6 and 1/2 of S and D are applied once at the end: with s = m + 4c + p = 6 S and d = p - m = 2 D per direction,
+//   grad_x = d_x s_y s_z / 72,   grad_y = s_x d_y s_z / 72,   grad_z = s_x s_y d_z / 72,   lap = s_x s_y s_z / 36 - 6 centre
+// (52 flops instead of 82 with the factors applied at every level).
 template <typename real, bool WALLS, bool IS_TEMP>
 __device__ __forceinline__ void stencil27(const StepArgs<real>& A, const Nbh<WALLS>& nb, const real* __restrict__ psi,
                                           real& centre, real grad[3], real& lap) {
-    const real c16 = real(1.0 / 6.0), c23 = real(2.0 / 3.0), half = real(0.5);
+    const real four = real(4);
     real SS[3], DSy[3], SDx[3];
 #pragma unroll
     for (int oz = -1; oz <= 1; ++oz) {
@@ -206,17 +209,18 @@ __device__ __forceinline__ void stencil27(const StepArgs<real>& A, const Nbh<WAL
                 v[ox + 1] = t;
             }
             if (oy == 0 && oz == 0) centre = v[1];
-            sx[oy + 1] = (v[0] + v[2]) * c16 + v[1] * c23;
-            dxv[oy + 1] = (v[2] - v[0]) * half;
+            sx[oy + 1] = (v[0] + v[2]) + four * v[1];
+            dxv[oy + 1] = v[2] - v[0];
         }
-        SS[oz + 1] = (sx[0] + sx[2]) * c16 + sx[1] * c23;
-        DSy[oz + 1] = (sx[2] - sx[0]) * half;
-        SDx[oz + 1] = (dxv[0] + dxv[2]) * c16 + dxv[1] * c23;
+        SS[oz + 1] = (sx[0] + sx[2]) + four * sx[1];
+        DSy[oz + 1] = sx[2] - sx[0];
+        SDx[oz + 1] = (dxv[0] + dxv[2]) + four * dxv[1];
     }
-    grad[0] = (SDx[0] + SDx[2]) * c16 + SDx[1] * c23;
-    grad[1] = (DSy[0] + DSy[2]) * c16 + DSy[1] * c23;
-    grad[2] = (SS[2] - SS[0]) * half;
-    lap = real(6) * (((SS[0] + SS[2]) * c16 + SS[1] * c23) - centre);
+    const real c72 = real(1.0 / 72.0);
+    grad[0] = c72 * ((SDx[0] + SDx[2]) + four * SDx[1]);
+    grad[1] = c72 * ((DSy[0] + DSy[2]) + four * DSy[1]);
+    grad[2] = c72 * (SS[2] - SS[0]);
+    lap = real(1.0 / 36.0) * ((SS[0] + SS[2]) + four * SS[1]) - real(6) * centre;
 }
 
 // ---------------------------------------------------------------------------------------------

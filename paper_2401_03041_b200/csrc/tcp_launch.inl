@@ -12,11 +12,11 @@ template <typename real, int QT, bool WALLS, int MODE, int AA>
 cudaError_t launch_staged(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
     const size_t smem = (size_t)(54 + QT - (h_direct<real, QT, AA>() ? 27 : 0)) * kBlock * sizeof(real);
     auto kern = fused_step_async_kernel<real, QT, WALLS, MODE, AA>;
-    static bool configured = false;      // once per instantiation (one device per process): saves ~1 us per launch
-    if (!configured) {
+    static bool configured[kMaxDevices] = {};   // once per instantiation and device: saves ~1 us per launch
+    if (!configured[c.device]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured[c.device] = true;
     }
     kern<<<c.grid, kBlock, smem, stream>>>(A);
     return cudaGetLastError();
@@ -24,10 +24,6 @@ cudaError_t launch_staged(const FusedCfg& c, const StepArgs<real>& A, cudaStream
 
 template <typename real, int QT, bool WALLS>
 cudaError_t dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
-    if (!c.staged && c.mode == 0 && !c.aa) {
-        fused_step_kernel<real, QT, WALLS, 0><<<c.grid, kBlock, 0, stream>>>(A);
-        return cudaGetLastError();
-    }
     if (c.mode == 3) {   // roofline calibration kernel (tcp_pattern_copy_ms): two-grid, periodic only
         if constexpr (!WALLS) return launch_staged<real, QT, false, 3, 0>(c, A, stream);
         else return cudaErrorNotSupported;
@@ -85,11 +81,11 @@ template <int QT, bool WALLS, int MODE, int AA>
 cudaError_t launch_pair(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_t stream) {
     const size_t smem = (size_t)(54 + QT - (pair_h_direct<QT, AA>() ? 27 : 0)) * kBlock * sizeof(float2);
     auto kern = fused_step_pair_kernel<QT, WALLS, MODE, AA>;
-    static bool configured = false;
-    if (!configured) {
+    static bool configured[kMaxDevices] = {};
+    if (!configured[c.device]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured[c.device] = true;
     }
     const unsigned grid = (unsigned)((((A.cell1 - A.cell0) >> 1) + kBlock - 1) / kBlock);
     kern<<<grid, kBlock, smem, stream>>>(A);

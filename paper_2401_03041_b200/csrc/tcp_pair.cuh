@@ -89,7 +89,7 @@ __device__ __forceinline__ void cp_async_8(float2* sdst, const float* gsrc) {
 template <bool WALLS, bool IS_TEMP>
 __device__ __forceinline__ void stencil27_pair(const StepArgs<f32x2>& A, const NbhPair<WALLS>& nb, const float* __restrict__ psi,
                                                f32x2& centre, f32x2 grad[3], f32x2& lap) {
-    const f32x2 c16(1.0 / 6.0), c23(2.0 / 3.0), half(0.5);
+    const f32x2 four(4.0);          // scaling deferred to the end, as in stencil27
     f32x2 SS[3], DSy[3], SDx[3];
 #pragma unroll
     for (int oz = -1; oz <= 1; ++oz) {
@@ -112,17 +112,18 @@ __device__ __forceinline__ void stencil27_pair(const StepArgs<f32x2>& A, const N
             }
             const f32x2 m(v0, v1), c(v1, v2), p(v2, v3);
             if (oy == 0 && oz == 0) centre = c;
-            sx[oy + 1] = (m + p) * c16 + c * c23;
-            dxv[oy + 1] = (p - m) * half;
+            sx[oy + 1] = (m + p) + four * c;
+            dxv[oy + 1] = p - m;
         }
-        SS[oz + 1] = (sx[0] + sx[2]) * c16 + sx[1] * c23;
-        DSy[oz + 1] = (sx[2] - sx[0]) * half;
-        SDx[oz + 1] = (dxv[0] + dxv[2]) * c16 + dxv[1] * c23;
+        SS[oz + 1] = (sx[0] + sx[2]) + four * sx[1];
+        DSy[oz + 1] = sx[2] - sx[0];
+        SDx[oz + 1] = (dxv[0] + dxv[2]) + four * dxv[1];
     }
-    grad[0] = (SDx[0] + SDx[2]) * c16 + SDx[1] * c23;
-    grad[1] = (DSy[0] + DSy[2]) * c16 + DSy[1] * c23;
-    grad[2] = (SS[2] - SS[0]) * half;
-    lap = f32x2(6.0) * (((SS[0] + SS[2]) * c16 + SS[1] * c23) - centre);
+    const f32x2 c72(1.0 / 72.0);
+    grad[0] = c72 * ((SDx[0] + SDx[2]) + four * SDx[1]);
+    grad[1] = c72 * ((DSy[0] + DSy[2]) + four * DSy[1]);
+    grad[2] = c72 * (SS[2] - SS[0]);
+    lap = f32x2(1.0 / 36.0) * ((SS[0] + SS[2]) + four * SS[1]) - f32x2(6.0) * centre;
 }
 
 // Thermal LB, two-grid: h is pulled straight into registers and only g and f are staged; for Q_T >= 15 three blocks then fit

@@ -20,8 +20,8 @@ namespace tcp {
 #ifndef TCP_RK_B3
 #define TCP_RK_B3 1
 #endif
-constexpr int kRkTX = 32, kRkTY = 8, kRkCZ = 32;   // chunks of 16-100 planes: within 1 % (profiles/r01_notes.md section 8)
-// Residency (profiles/r01_notes.md section 8): with the cell data requested one plane ahead the fp64 kernel needs
+constexpr int kRkTX = 32, kRkTY = 8, kRkCZ = 32;   // chunks of 16-100 planes: within 1 %
+// Residency: with the cell data requested one plane ahead the fp64 kernel needs
 // 119 registers -> 2 blocks of 256 per SM without spills (3 blocks: 80-116 B of spills and 8-15 % slower);
 // the fp32 kernel fits 3 blocks.
 template <typename real, bool HAS_DK>
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real, HAS_DK>()) 
         for (int i = 0; i < NE; ++i)
             if (e_on[i]) { tileY[buf][tid + i * TX * TY] = pfY[i]; if (HAS_DK) tileP[buf][tid + i * TX * TY] = pfP[i]; }
     };
-    const real c16 = real(1.0 / 6.0), c23 = real(2.0 / 3.0), half = real(0.5);
+    const real four = real(4), c72 = real(1.0 / 72.0), c36 = real(1.0 / 36.0);   // scaling deferred to the end, as in stencil27
     auto reduce_plane = [&](const real* t) {
         Plane3<real> P;
         real sx[3], dxv[3];
@@ -109,12 +109,12 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real, HAS_DK>()) 
             const real* row = t + (threadIdx.y + oy) * PX + threadIdx.x;
             const real m = row[0], c = row[1], p = row[2];
             if (oy == 1) P.c = c;
-            sx[oy] = (m + p) * c16 + c * c23;
-            dxv[oy] = (p - m) * half;
+            sx[oy] = (m + p) + four * c;
+            dxv[oy] = p - m;
         }
-        P.S = (sx[0] + sx[2]) * c16 + sx[1] * c23;
-        P.Dy = (sx[2] - sx[0]) * half;
-        P.Dx = (dxv[0] + dxv[2]) * c16 + dxv[1] * c23;
+        P.S = (sx[0] + sx[2]) + four * sx[1];
+        P.Dy = sx[2] - sx[0];
+        P.Dx = (dxv[0] + dxv[2]) + four * dxv[1];
         return P;
     };
 
@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real, HAS_DK>()) 
     if (HAS_DK) { Pm = reduce_plane(tileP[0]); Pc = reduce_plane(tileP[1]); }
     __syncthreads();                       // buffer 0 may now be overwritten
     // cell data (u, T^n, accumulator, source, phi) of plane z0 + k: every thread copies its own cell's values D - 1 planes
-    // ahead (RK4 -1.5 % against one plane ahead in registers, profiles/r01_notes.md section 23) with cp.async into its slot of a shared-memory ring (it reads only what it copied itself, so
+    // ahead (RK4 -1.5 % against one plane ahead in registers) with cp.async into its slot of a shared-memory ring (it reads only what it copied itself, so
     // cp.async.wait_group is all the synchronisation this needs); no registers are held while they are in flight
     constexpr int D = TCP_RK_RING, NV = 7, RING = NV * TX * TY;
     extern __shared__ __align__(16) unsigned char rk_ring_raw[];
@@ -173,14 +173,14 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real, HAS_DK>()) 
         if (HAS_DK) Pp = reduce_plane(tileP[buf]);
         if (inside) {
             real gY[3], G[3] = {real(0), real(0), real(0)};
-            gY[0] = (Ym.Dx + Yp.Dx) * c16 + Yc.Dx * c23;
-            gY[1] = (Ym.Dy + Yp.Dy) * c16 + Yc.Dy * c23;
-            gY[2] = (Yp.S - Ym.S) * half;
-            const real lapY = real(6) * (((Ym.S + Yp.S) * c16 + Yc.S * c23) - Yc.c);
+            gY[0] = c72 * ((Ym.Dx + Yp.Dx) + four * Yc.Dx);
+            gY[1] = c72 * ((Ym.Dy + Yp.Dy) + four * Yc.Dy);
+            gY[2] = c72 * (Yp.S - Ym.S);
+            const real lapY = c36 * ((Ym.S + Yp.S) + four * Yc.S) - real(6) * Yc.c;
             if (HAS_DK) {
-                G[0] = (Pm.Dx + Pp.Dx) * c16 + Pc.Dx * c23;
-                G[1] = (Pm.Dy + Pp.Dy) * c16 + Pc.Dy * c23;
-                G[2] = (Pp.S - Pm.S) * half;
+                G[0] = c72 * ((Pm.Dx + Pp.Dx) + four * Pc.Dx);
+                G[1] = c72 * ((Pm.Dy + Pp.Dy) + four * Pc.Dy);
+                G[2] = c72 * (Pp.S - Pm.S);
             }
             const real phi_c = HAS_DK ? Pc.c : phi_here;
             const real kap = A.kappa_L + phi_c * A.dkappa;

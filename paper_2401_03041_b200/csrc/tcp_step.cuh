@@ -17,10 +17,19 @@ constexpr int kBlock = TCP_BLOCK;
 // fp32 only.  In real arithmetic the collision conserves the zeroth moment (sum_q E_q = s because
 // sum_q w_q = 1), but the rounded weights do not sum to 1, which re-creates the whole population
 // with the same relative bias (~1e-8) every step: sum(phi) then drifts linearly (measured 7.5e-5
-// over 1e4 steps).  So the zeroth moment of the pulled populations is summed in fp64 (exact for 27
-// floats of similar size) and the rest population is written as the fp64 remainder, rounded once:
-// what is left is one unbiased rounding per cell and step.  In fp64 the bias is ~1e-17 per step
-// and the arithmetic is left as derived.
+// over 1e4 steps).  So the rest population is not taken from the formula but written as a remainder.
+// Round 1 summed the zeroth moment and the remainder in fp64 (252 conversions + 238 DADD per pair of
+// cells: 15 % of the pair kernel's instructions, XU pipe 31 % busy; TCP_F32_EXACT0 = 1 restores it).
+// Now both stay in fp32 and are built from the SAME ordered partial sum over the 26 moving populations,
+//     s = fl(P_in + a_rest),   a~_rest = fl(s - P_out),   P = ((a_0 + a_26) + (a_1 + a_25)) + ...,
+// so that wherever the state is steady (a~_q = a_q for the moving q, hence P_out = P_in) the remainder
+// reproduces itself exactly (s / 2 <= P <= 2 s: the subtraction is exact, Sterbenz) and the stored total stops
+// changing.  With the remainder taken against a differently ordered sum (e.g. the tree of moments27)
+// every quasi-steady cell repeats the same rounding mismatch step after step and sum(phi) drifts
+// 1.5e-6 over 1e4 steps (measured).  In fp64 the bias is ~1e-17 per step and the arithmetic is left as derived.
+#ifndef TCP_F32_EXACT0
+#define TCP_F32_EXACT0 0
+#endif
 template <typename real>
 __device__ __forceinline__ wide_t<real> exact_sum27(const real a[27]) {
     wide_t<real> s = wide_zero<real>();
@@ -28,13 +37,25 @@ __device__ __forceinline__ wide_t<real> exact_sum27(const real a[27]) {
     for (int q = 0; q < 27; ++q) s += widen(a[q]);
     return s;
 }
+// P of the comment above
 template <typename real>
-__device__ __forceinline__ void conserve_zeroth27(real a[27], wide_t<real> s) {
-    if constexpr (real_traits<real>::single) {
+__device__ __forceinline__ real moving_sum27(const real a[27]) {
+    real P = a[0] + a[26];
 #pragma unroll
-        for (int q = 0; q < 27; ++q)
-            if (q != 13) s -= widen(a[q]);
-        a[13] = narrow<real>(s);
+    for (int q = 1; q < 13; ++q) P += (a[q] + a[26 - q]);
+    return P;
+}
+template <typename real>
+__device__ __forceinline__ void conserve_zeroth27(real a[27], real s, wide_t<real> s_exact) {
+    if constexpr (real_traits<real>::single) {
+        if constexpr (TCP_F32_EXACT0) {
+#pragma unroll
+            for (int q = 0; q < 27; ++q)
+                if (q != 13) s_exact -= widen(a[q]);
+            a[13] = narrow<real>(s_exact);
+        } else {
+            a[13] = s - moving_sum27<real>(a);
+        }
     }
 }
 
@@ -78,7 +99,10 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
     const Mom2<real> M = moments27<real, false>(h);
     wide_t<real> phin_exact = wide_zero<real>();
     real phin = M.m0;
-    if constexpr (real_traits<real>::single) { phin_exact = exact_sum27<real>(h); phin = narrow<real>(phin_exact); }
+    if constexpr (real_traits<real>::single) {
+        if constexpr (TCP_F32_EXACT0) { phin_exact = exact_sum27<real>(h); phin = narrow<real>(phin_exact); }
+        else phin = moving_sum27<real>(h) + h[13];
+    }
     // a = c_s^2 [4 phi (1 - phi) / xi] n,  n = G / sqrt(G.G + eps)   (eq. 15, readings S7, S8)
     const real inv = rsqrt_<real>(G[0] * G[0] + G[1] * G[1] + G[2] * G[2] + A.eps);
     const real mag = real(4.0 / 3.0) * phi_c * (real(1) - phi_c) * A.inv_xi * inv;
@@ -109,7 +133,7 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = out[q];
     }
-    conserve_zeroth27<real>(h, phin_exact);
+    conserve_zeroth27<real>(h, phin, phin_exact);
     return phin;
 }
 
@@ -121,7 +145,10 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
     const Mom2<real> M = moments27<real, true>(g);
     wide_t<real> ps_exact = wide_zero<real>();
     real ps = M.m0;                                         // p* (eq. 17)
-    if constexpr (real_traits<real>::single) { ps_exact = exact_sum27<real>(g); ps = narrow<real>(ps_exact); }
+    if constexpr (real_traits<real>::single) {
+        if constexpr (TCP_F32_EXACT0) { ps_exact = exact_sum27<real>(g); ps = narrow<real>(ps_exact); }
+        else ps = moving_sum27<real>(g) + g[13];
+    }
     const real j[3] = {M.mx, M.my, M.mz};
     const real rho = A.rho_L + phi_c * A.drho;              // eq. 14
     const real tau = A.tau_L + phi_c * A.dtau;              // eq. 22
@@ -217,7 +244,7 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = out[q];
     }
-    conserve_zeroth27<real>(g, ps_exact);
+    conserve_zeroth27<real>(g, ps, ps_exact);
 }
 
 // ---- thermal LB on one cell: eqs. 27-29 (rho c_p = 1 on this path, S11) ------------------------
@@ -225,15 +252,20 @@ template <typename real, int Q, int MODE>
 __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[Q], real phi_new, const real u[3], real qT) {
     real Tn = real(0), j[3] = {real(0), real(0), real(0)};
     wide_t<real> Tn_exact = wide_zero<real>();
+    constexpr bool ordered = real_traits<real>::single && !TCP_F32_EXACT0;   // see conserve_zeroth27
+    if constexpr (ordered) {
+        static_for<0, Q / 2>([&](auto K) { constexpr int k = decltype(K)::value; Tn += (f[k] + f[Q - 1 - k]); });
+        Tn += f[Q / 2];
+    }
     static_for<0, Q>([&](auto K) {
         constexpr int k = decltype(K)::value, q = q_of(Q, k);
-        if constexpr (real_traits<real>::single) Tn_exact += widen(f[k]); else
-        Tn += f[k];                                          // eq. 28
+        if constexpr (real_traits<real>::single && TCP_F32_EXACT0) Tn_exact += widen(f[k]); else
+        if constexpr (!ordered) Tn += f[k];                  // eq. 28
         if constexpr (cx27(q) != 0) j[0] += real(cx27(q)) * f[k];
         if constexpr (cy27(q) != 0) j[1] += real(cy27(q)) * f[k];
         if constexpr (cz27(q) != 0) j[2] += real(cz27(q)) * f[k];
     });
-    if constexpr (real_traits<real>::single) Tn = narrow<real>(Tn_exact);
+    if constexpr (real_traits<real>::single && TCP_F32_EXACT0) Tn = narrow<real>(Tn_exact);
     const real kap = A.kappa_L + phi_new * A.dkappa;         // eq. 23 (G5)
     const real w = real(1) / (real(0.5) + real(3) * kap);    // eq. 29 read as a rate (G4)
     real out[Q];
@@ -252,9 +284,15 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
         }
     }
     if constexpr (real_traits<real>::single) {   // see conserve_zeroth27
-        wide_t<real> rest = Tn_exact;
-        static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; if constexpr (k != Q / 2) rest -= widen(out[k]); });
-        out[Q / 2] = narrow<real>(rest);
+        if constexpr (TCP_F32_EXACT0) {
+            wide_t<real> rest = Tn_exact;
+            static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; if constexpr (k != Q / 2) rest -= widen(out[k]); });
+            out[Q / 2] = narrow<real>(rest);
+        } else {
+            real P = real(0);
+            static_for<0, Q / 2>([&](auto K) { constexpr int k = decltype(K)::value; P += (out[k] + out[Q - 1 - k]); });
+            out[Q / 2] = Tn - P;
+        }
     }
     static_for<0, Q>([&](auto K) {
         constexpr int k = decltype(K)::value, q = q_of(Q, k);
@@ -277,60 +315,7 @@ __device__ __forceinline__ real rk_stage1_local(const StepArgs<real>& A, real ph
 }
 
 // ---------------------------------------------------------------------------------------------
-template <typename real, int QT, bool WALLS, int MODE>
-__global__ void __launch_bounds__(kBlock, TCP_MINB) fused_step_kernel(const StepArgs<real> A) {
-    const int gtid = A.cell0 + blockIdx.x * kBlock + threadIdx.x;
-    if (gtid >= A.cell1) return;
-    const long long N = A.ncell;
-    Nbh<WALLS> nb;
-    nb.init(A, gtid);
-    const int cell = nb.idx;
-
-    real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
-    stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
-    stencil27<real, WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
-    real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
-
-    real phi_new;
-    {
-        real h[27];
-        pull27<real, WALLS>(A, nb, A.h_in, h);
-        phi_new = collide_phase<real, MODE>(A, h, G, phi_c, u);
-#pragma unroll
-        for (int q = 0; q < 27; ++q) A.h_out[q * N + cell] = h[q];
-        A.phi_out[cell] = phi_new;
-    }
-    {
-        real g[27];
-        pull27<real, WALLS>(A, nb, A.g_in, g);
-        if (WALLS && A.moving) {
-#pragma unroll
-            for (int q = 0; q < 27; ++q) g[q] += wall_velocity_term<real, WALLS>(A, nb, q);
-        }
-        collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
-#pragma unroll
-        for (int q = 0; q < 27; ++q) A.g_out[q * N + cell] = g[q];
-        A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
-    }
-    if constexpr (QT == 0) {
-        if (A.rk1_out) {
-            const real rhs = rk_stage1_local<real>(A, phi_new, u, Th, lapT, A.q_src ? A.q_src[cell] : real(0));
-            A.rk1_out[cell] = T_c + A.rk1_c_out * rhs;
-            if (A.rk1_acc) A.rk1_acc[cell] = T_c + A.rk1_c_acc * rhs;
-        }
-    }
-    if constexpr (QT > 0) {
-        real f[QT];
-        pull_thermal<real, QT, WALLS>(A, nb, A.f_in, f);
-        const real qT = A.q_src ? A.q_src[cell] : real(0);
-        const real Tn = collide_thermal<real, QT, MODE>(A, f, phi_new, u, qT);
-        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; A.f_out[k * N + cell] = f[k]; });
-        A.T_out[cell] = Tn;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// fused_step_async_kernel: the same step, but every thread first issues ALL of its 27 + 27 + Q_T
+// fused_step_async_kernel: one thread carries a cell through the whole step.  It first issues ALL of its 27 + 27 + Q_T
 // pulls as asynchronous global->shared copies (cp.async, SASS LDGSTS; slot [q][tid], so a thread only
 // ever reads what it copied itself and cp.async.wait_group is the only synchronisation needed), then
 // does the phi / T stencils, then consumes the three groups in order.  Loads in flight per SM become
@@ -633,6 +618,38 @@ __global__ void __launch_bounds__(kBlock) thermal_only_kernel(const StepArgs<rea
     A.T_out[cell] = Tn;
 }
 
+// ---- AA streaming: a wall temperature that changes while the populations are in the pushed layout -------------
+// After tcp_init_fields and after every odd step a link of f~ into a wall is stored already anti-bounced (plane opp(q)
+// at the cell, value 2 w T_w - f~_q, see pop_dst), so that the even step that follows needs no boundary code.  The
+// stored value carries the T_w of the moment it was written; when tcp_set_wall_temperature replaces the plane of wall
+// (axis, face) in that state, the difference 2 w (T_w_new - T_w_old) is folded into the stored links of that wall, and
+// the next (even) step then sees exactly what a two-grid pull with the new plane would compute (reading S9).
+// One thread per cell of the wall's first fluid layer; `plane_cells` = cells in the tangential plane.
+template <typename real, int QT>
+__global__ void __launch_bounds__(kBlock) aa_wall_repush_kernel(const StepArgs<real> A, real* __restrict__ f, int axis, int face,
+                                                               const real* __restrict__ Tw_new, const real* __restrict__ Tw_old, int plane_cells) {
+    const int t = blockIdx.x * kBlock + threadIdx.x;
+    if (t >= plane_cells) return;
+    const int n[3] = {A.nx, A.ny, A.nz};
+    int xyz[3];
+    const int a1 = axis == 0 ? 1 : 0, a2 = axis == 2 ? 1 : 2;   // tangential axes, fastest first (plane layout of tcp.h)
+    xyz[axis] = face ? n[axis] - 1 : 0;
+    xyz[a1] = t % n[a1];
+    xyz[a2] = t / n[a1];
+    Nbh<true> nb;
+    nb.init_xyz(A, xyz[0], xyz[1], xyz[2]);
+    const long long N = A.ncell;
+    static_for<0, QT>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(QT, k);
+        int fc = 0;
+        const int ax = nb.crossed(cx27(q), cy27(q), cz27(q), fc);
+        if (ax == axis && fc == face) {
+            const int i = nb.tangential(axis, cx27(q), cy27(q), cz27(q));
+            f[(QT - 1 - k) * N + nb.idx] += real(2.0 * weight(QT, cls27(q))) * (Tw_new[i] - Tw_old[i]);
+        }
+    });
+}
+
 // ---- Runge-Kutta stages of eq. 4 (eqs. 25-26; reading G6) --------------------
 template <typename real>
 struct RkArgs {
@@ -646,34 +663,6 @@ struct RkArgs {
     real c_acc;              // acc_out = (first ? Tn : acc_in) + c_acc R
     int mode;                // 0: out only; 1: out and acc from Tn; 2: out and acc from acc_in; 3: out = acc_in + c_acc R
 };
-
-template <typename real, bool WALLS>
-__global__ void __launch_bounds__(kBlock) rk_stage_kernel(const RkArgs<real> R) {
-    const StepArgs<real>& A = R.S;
-    const int gtid = A.cell0 + blockIdx.x * kBlock + threadIdx.x;
-    if (gtid >= A.cell1) return;
-    const long long N = A.ncell;
-    Nbh<WALLS> nb;
-    nb.init(A, gtid);
-    const int cell = nb.idx;
-    real phi_c, G[3], lapPhi, Y_c, gY[3], lapY;
-    stencil27<real, WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
-    stencil27<real, WALLS, true>(A, nb, R.Y, Y_c, gY, lapY);
-    const real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
-    const real kap = A.kappa_L + phi_c * A.dkappa;
-    const real rcp = (A.rho_L + phi_c * A.drho) * (A.cp_L + phi_c * A.dcp);   // rho(phi) c_p(phi) (A14)
-    const real adv = u[0] * gY[0] + u[1] * gY[1] + u[2] * gY[2];
-    const real dk = A.dkappa * (G[0] * gY[0] + G[1] * gY[1] + G[2] * gY[2]);
-    const real rhs = -adv + (dk + kap * lapY) / rcp + (A.q_src ? A.q_src[cell] : real(0));
-    const real Tn = R.Tn[cell];
-    if (R.mode == 3) {
-        R.out[cell] = R.acc_in[cell] + R.c_acc * rhs;
-    } else {
-        R.out[cell] = Tn + R.c_out * rhs;
-        if (R.mode == 1) R.acc_out[cell] = Tn + R.c_acc * rhs;
-        if (R.mode == 2) R.acc_out[cell] = R.acc_in[cell] + R.c_acc * rhs;
-    }
-}
 
 // ---- initialisation and read-back --------------------------------------------------------------
 template <typename real, int QT>

@@ -61,13 +61,37 @@ def assert_parity_f64(got, want, tol=1e-10):
         assert err <= tol, f"{name}: max-abs error {err:.3e} > {tol:.1e}"
 
 
-def assert_parity_f32(got, want, rel=1e-5):
-    """north_star: fp32 variant <= 1e-5 relative (to the field's own scale: max |oracle|; for u and p,
-    whose scale can be ~1e-6 in a quiescent set-up, the scale is floored so that round-off of the
-    O(1) populations they are differences of still counts as relative error of those populations)."""
-    floors = dict(phi=1.0, u=1.0, p=1.0 / 3.0, T=1.0)
+def fp32_errors(got, want):
+    """name -> (max-abs error, max |oracle|, their ratio or None): the TRUE relative errors, no floor."""
+    out = {}
     for name, g, w in zip(NAMES, got, want):
+        err = float(np.abs(np.asarray(g, dtype=np.float64) - w).max())
+        scale = float(np.abs(w).max())
+        out[name] = (err, scale, err / scale if scale > 0 else None)
+    return out
+
+
+def assert_parity_f32(got, want, sigma=0.0, rel=1e-5, label=""):
+    """north_star: the fp32 variant matches the fp64 oracle to <= 1e-5 relative.  Relative means
+    max |gpu - oracle| / max |oracle| per field, with NO floor on the scale; the true figures are printed
+    (pytest -rP shows them) and tabulated in DESIGN.md section 7.
+
+    phi and T are O(1) fields and are held to the literal bar.  u and p are held to it too wherever the flow is
+    stronger than what fp32 can resolve at all: a 24-bit phi carries an absolute rounding of ~3e-8, the Laplacian in
+    mu_phi multiplies it by ~6 and by k = 1.5 sigma xi, and F_s = mu_phi grad phi with |grad phi| <= 1 / xi turns that into
+    a force noise of ~3e-7 sigma per step and cell, whatever the size of u.  Measured on the GPU:
+    |u_f32 - u_oracle| <= 1.2e-6 sigma_ref and |p_f32 - p_oracle| <= 4e-7 sigma_ref in every set-up, from 10 to 1000
+    steps.  So u (p) passes if its error is below 1e-5 max|u| OR below the noise floor 2e-6 sigma_ref (1e-6 sigma_ref);
+    `sigma` = sigma_ref of the run (0: no floor at all).  An fp32-only velocity bug of a few per cent of u cannot hide
+    behind these floors unless u itself is below 1e-4 sigma."""
+    floors = dict(phi=0.0, u=2e-6 * sigma, p=1e-6 * sigma, T=0.0)
+    errs = fp32_errors(got, want)
+    print(f"fp32 true errors {label}: " + "  ".join(
+        f"{n}: {e:.2e} / {sc:.2e} = {('%.1e' % r) if r is not None else 'n/a'}" for n, (e, sc, r) in errs.items()))
+    for name, g in zip(NAMES, got):
         assert np.all(np.isfinite(g)), f"{name} has non-finite values"
-        scale = max(np.abs(w).max(), floors[name])
-        err = np.abs(g.astype(np.float64) - w).max() / scale
-        assert err <= rel, f"{name}: relative error {err:.3e} > {rel:.1e}"
+        err, scale, _ = errs[name]
+        bar = max(rel * scale, floors[name])
+        if scale == 0.0:
+            bar = max(bar, 1e-7)            # an identically zero oracle field (isothermal T): absolute round-off only
+        assert err <= bar, f"{name}: error {err:.3e} > max({rel:.0e} x {scale:.3e}, noise floor {floors[name]:.1e})"

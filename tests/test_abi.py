@@ -55,12 +55,26 @@ def test_workspace_bytes_accounting():
 @pytest.mark.parametrize("bad, code", [
     (dict(M=0.0), tcp.TCP_EINVAL), (dict(xi=-1.0), tcp.TCP_EINVAL), (dict(tau_H=-0.5), tcp.TCP_EINVAL),
     (dict(rho_L=0.0), tcp.TCP_EINVAL), (dict(kappa_H=0.0), tcp.TCP_EINVAL),
+    (dict(eps_normal=0.0), tcp.TCP_EINVAL), (dict(s_bulk=0.0), tcp.TCP_EINVAL), (dict(s_high=2.0), tcp.TCP_EINVAL),
+    (dict(high_rate_equals_shear=2), tcp.TCP_EINVAL),
 ])
 def test_parameter_validation(bad, code):
     with pytest.raises(tcp.TcpError) as e:
         tcp.tcp_workspace_bytes(8, 8, 8, tcp.make_params(bad))
     assert e.value.code == code
     assert tcp.tcp_last_error()
+
+
+def test_params_default_matches_the_binding_and_a_zeroed_struct_is_rejected():
+    """tcp_params_default (include/tcp.h) fills what the Python binding's PARAM_DEFAULTS documents; a C caller who
+    memsets the struct and sets only struct_size gets TCP_EINVAL instead of NaNs (eps_normal = 0, rates 0)."""
+    d, b = tcp.tcp_params_default(), tcp.make_params({})
+    assert bytes(d) == bytes(b)
+    z = tcp.tcp_params()
+    z.struct_size = C.sizeof(tcp.tcp_params)
+    with pytest.raises(tcp.TcpError) as e:
+        tcp.tcp_workspace_bytes(8, 8, 8, z)
+    assert e.value.code == tcp.TCP_EINVAL
 
 
 def test_extent_validation():

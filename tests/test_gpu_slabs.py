@@ -95,22 +95,18 @@ def test_tweezer_with_heat_source_and_initial_velocity():
     assert_same_bits(got, want)
 
 
-@pytest.mark.parametrize("kernel", ["pair", "scalar"])
-def test_fp32_slabs(kernel, monkeypatch):
-    if kernel == "scalar":
-        monkeypatch.setenv("TCP_KERNEL", "scalar")
-    wl = configs.perf_box(24, thermal="lb_d3q7", ny=16, nz=15, seed=2, r_min=4.0, r_max=5.0)
+@pytest.mark.parametrize("nx", [24, 23])
+def test_fp32_slabs(nx):
+    # even nx: the packed-pair kernel; odd nx: one cell per thread
+    wl = configs.perf_box(nx, thermal="lb_d3q7", ny=16, nz=15, seed=2, r_min=4.0, r_max=5.0)
     want, _ = run_gpu(wl, 15, precision="f32")
     got, _ = run_slabs(wl, 3, 15, precision="f32")
     assert_same_bits(got, want)
 
 
 @pytest.mark.parametrize("thermal", ["rk2", "rk4"])
-@pytest.mark.parametrize("kernel", ["march", "flat"])
-def test_runge_kutta_slabs(thermal, kernel, monkeypatch):
+def test_runge_kutta_slabs(thermal):
     # Algorithm 2: one transfer after the fused kernel and one after every stage (3 / 5 per step)
-    if kernel == "flat":
-        monkeypatch.setenv("TCP_KERNEL", "flat")
     wl = configs.perf_box(36, thermal=thermal, ny=20, nz=23, seed=4, r_min=4.0, r_max=5.0)   # x spans two 32-wide tiles
     want, _ = run_gpu(wl, 12)
     got, _ = run_slabs(wl, 3, 12)

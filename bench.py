@@ -63,10 +63,27 @@ def hbm_peak():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+NOMINAL_HBM_GBS = 8000.0     # B200 HBM3e data-sheet figure; context only, the roofline denominator is the measured copy peak
+
+
 def recorded_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu capture
+    (profiles/traffic.json: bytes, the commit that was profiled, the ncu command); None if that variant was not captured."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(path):
-        return json.load(open(path)).get(key)
+        e = json.load(open(path)).get(key)
+        if isinstance(e, dict):
+            return e.get("bytes")
+        return e
+    return None
+
+
+def traffic_provenance(key):
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        e = json.load(open(path)).get(key)
+        if isinstance(e, dict):
+            return {k: e.get(k) for k in ("commit", "command", "profile")}
     return None
 
 
@@ -159,6 +176,41 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def timed_variant(tcp, n, thermal, prec, streaming, warmup, steps, device_index, peak):
+    """One short device-timed run of another row of BASELINE configs[4] (W >= 3 warm-up steps, K >= 20 timed, CUDA
+    events of the library around its own launches, clocks sampled during the timed region)."""
+    es = 8 if prec == "f64" else 4
+    tdt = torch.float64 if prec == "f64" else torch.float32
+    wl = W.perf_box(n, thermal=thermal, device="cuda")
+    sim = tcp.Simulation(n, n, n, dict(wl.params, precision=prec, streaming=streaming))
+    sim.init_fields(wl.phi.to(tdt).contiguous(), None, wl.T.to(tdt).contiguous())
+    del wl
+    sim.step(max(warmup, 3))
+    torch.cuda.synchronize()
+    sampler = ClockSampler(device_index)
+    sampler.start()
+    l0 = sim.launches
+    sim.step(steps)
+    ms = sim.last_step_ms() / steps
+    launches = sim.launches - l0
+    clocks = sampler.stop()
+    finite = bool(torch.isfinite(sim.read_fields_device()[0]).all().item())
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+    bpc = step_values_per_cell(thermal) * es
+    gbs = bpc * n ** 3 / (ms * 1e-3) / 1e9
+    return {"workload": f"perf_box {n}^3", "thermal": thermal, "dtype": prec, "streaming": streaming, "steps": steps,
+            "warmup": max(warmup, 3), "ms_per_step": ms, "mlups": n ** 3 / (ms * 1e-3) / 1e6, "step_bytes_per_cell": bpc,
+            "achieved_gbs": gbs, "frac": gbs / peak, "frac_of_nominal": gbs / NOMINAL_HBM_GBS, "gpu_launches": launches,
+            "clocks": clocks, "finite": finite}
+
+
+VARIANTS = [(400, "lb_d3q15", "f64", "two_grid"), (400, "lb_d3q19", "f64", "two_grid"), (400, "lb_d3q27", "f64", "two_grid"),
+            (400, "rk2", "f64", "two_grid"), (400, "rk4", "f64", "two_grid"), (400, "lb_d3q7", "f64", "aa"),
+            (512, "lb_d3q7", "f32", "two_grid"), (512, "rk2", "f32", "two_grid"), (256, "lb_d3q7", "f64", "two_grid")]
+
+
 def run_ours(args):
     import paper_2401_03041_b200 as tcp
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -180,6 +232,8 @@ def run_ours(args):
     params = dict(wl.params, precision=prec, streaming=args.streaming)
     sim = tcp.Simulation(n, n, n, params)
     phi_d, T_d = wl.phi.to(tdt).contiguous(), wl.T.to(tdt).contiguous()
+    wl_notes, wl_fields = wl.notes, (wl.phi, wl.T)
+    wl.phi = wl.T = None
     sim.init_fields(phi_d, None, T_d)
 
     def barrier():
@@ -211,6 +265,16 @@ def run_ours(args):
     if rank == 0 and args.streaming == "two_grid" and QT[thermal]:   # calibrated for the one-kernel (thermal LB) step only
         sim.pattern_copy_ms(3)
         pattern_ms = sim.pattern_copy_ms(max(5, min(args.steps, 20)))
+    # ---- sustained figure: the same kernel for >= 3 s after the K-step region, with its own clock record.  The K-step
+    # region of the default line is a 0.2-0.6 s burst at boost clocks; a long run sits on the 1000 W power cap.
+    sustained = None
+    if rank == 0 and args.sustain_s > 0:
+        n_sus = max(args.steps, int(args.sustain_s * 1e3 / (ms / args.steps)) + 1)
+        sampler2 = ClockSampler(local)
+        sampler2.start()
+        sim.step(n_sus)
+        sus_ms = sim.last_step_ms() / n_sus
+        sustained = {"steps": n_sus, "ms_per_step": sus_ms, "mlups": N / (sus_ms * 1e-3) / 1e6, "clocks": sampler2.stop()}
     phi_chk = sim.read_fields_device()[0]
     finite = bool(torch.isfinite(phi_chk).all().item())
     sum_drift = abs(float(phi_chk.double().sum().item()) - float(phi_d.double().sum().item())) / float(phi_d.double().sum().item())
@@ -236,8 +300,14 @@ def run_ours(args):
         dt_max = max_over_ranks(dt * 1e3, dist)
         e2e = {"value": aggregate_mlups(N, args.steps, world, dt_max), "unit": "MLUPS",
                "h2d_bytes_per_step": 5 * N * es / args.steps, "d2h_bytes_per_step": 6 * N * es / args.steps,
-               "note": f"tcp_init_fields(host) + tcp_step({args.steps}) + tcp_read_fields(host), pinned host buffers"}
+               "steps": args.steps, "h2d_bytes": 5 * N * es, "d2h_bytes": 6 * N * es, "wall_s": dt_max * 1e-3,
+               "note": f"tcp_init_fields(host) + tcp_step({args.steps}) + tcp_read_fields(host), pinned host buffers; the one-off "
+                       f"copies of the initial and final fields are amortised over the {args.steps} steps of the call, so this "
+                       "figure depends on the step count (state it when quoting)"}
         del hp, hT, hu, o_phi, o_T, o_p, o_u
+    sim.close()
+    del sim, phi_d, T_d, wl_fields
+    torch.cuda.empty_cache()
 
     if rank != 0:
         if dist:
@@ -250,30 +320,45 @@ def run_ours(args):
     if QT[thermal]:
         k_ms = kernel_ms / args.steps                      # one fused kernel per step
         achieved = fused_bytes / (k_ms * 1e-3) / 1e9
-        kname = ("fused_step_pair_kernel" if prec == "f32" and os.environ.get("TCP_KERNEL") != "scalar" else "fused_step_async_kernel")
+        kname = "fused_step_pair_kernel" if prec == "f32" and n % 2 == 0 else "fused_step_async_kernel"
     else:
         k_ms = kernel_ms / args.steps
         achieved = step_bytes / (k_ms * 1e-3) / 1e9        # whole step (fused kernel + RK stages)
         kname = "fused_step_async_kernel + rk_stage_march_kernel (whole step)"
+    alg_bytes = fused_bytes if QT[thermal] else step_bytes
+    tkey = f"{thermal}_{prec}_{n}" + ("_aa" if args.streaming == "aa" else "")
+    if sustained is not None:
+        sus_gbs = alg_bytes / (sustained["ms_per_step"] * 1e-3) / 1e9
+        sustained.update({"achieved": sus_gbs, "frac": sus_gbs / peak, "frac_of_nominal": sus_gbs / NOMINAL_HBM_GBS})
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": recorded_traffic(f"{thermal}_{prec}_{n}"), "kernel": kname, "peak_source": peak_src,
-                "algorithmic_bytes_per_cell": (fused_bytes if QT[thermal] else step_bytes) / N,
+                "frac_of_nominal": achieved / NOMINAL_HBM_GBS, "nominal_peak": NOMINAL_HBM_GBS,
+                "traffic": recorded_traffic(tkey), "traffic_source": traffic_provenance(tkey), "kernel": kname, "peak_source": peak_src,
+                "algorithmic_bytes_per_cell": alg_bytes / N,
                 "kernel_ms": k_ms,
+                # the same kernel over >= 3 s directly after the timed region (power-capped clocks): the figure to quote
+                # for production runs; `frac` above is the K-step region the contract times
+                "sustained": sustained,
                 # what a no-arithmetic kernel with the fused kernel's pulls, staging and stores reaches on this GPU
                 "pattern_copy": None if pattern_ms is None else {"ms": pattern_ms, "gbs": fused_bytes / (pattern_ms * 1e-3) / 1e9,
                                                                   "frac_of_peak": fused_bytes / (pattern_ms * 1e-3) / 1e9 / peak}}
+    variants = None
+    if world == 1 and not args.no_variants and (n, thermal, prec, args.streaming) == (400, "lb_d3q7", "f64", "two_grid"):
+        # the other rows of BASELINE configs[4] under the same clock (the headline above stays the metric's line)
+        variants = [timed_variant(tcp, *v, args.warmup, max(args.variant_steps, 20), local, peak) for v in VARIANTS]
     cpu = None
     if not args.no_cpu:
         v, _, cores, sample = oracle_throughput(thermal)
-        cpu = {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample}
+        cpu = {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample,
+               "note": "the parity oracle as it stands (dense K(u) + Gaussian elimination per cell): a correctness reference, not a performance baseline"}
     line = {"metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": prec, "data": "synthetic",
             "config": {"workload": f"perf_box {n}^3 periodic (BASELINE configs[4]), hydro D3Q27 CM, phase D3Q27, thermal {thermal}, streaming {args.streaming}",
                        "cells_per_gpu": N, "parallelism": "replicas" if world > 1 else "single GPU",
                        "l2": f"working set {step_bytes / 1e9:.1f} GB per step >> 126 MB L2, no flush needed",
-                       "notes": wl.notes},
+                       "e2e_steps": args.steps, "notes": wl_notes},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "variants": variants,
             "checks": {"finite": finite, "sum_phi_rel_drift": sum_drift}}
     print(json.dumps(line), flush=True)
     if dist:
@@ -385,6 +470,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-size", type=int, default=64)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-variants", action="store_true", help="skip the short runs of the other configs[4] rows")
+    ap.add_argument("--variant-steps", type=int, default=25)
+    ap.add_argument("--sustain-s", type=float, default=3.0, help="seconds of steps after the timed region for roofline.sustained (0: skip)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="per-variant / per-size table (configs[4]); one JSON line each")
     ap.add_argument("--sweep-sizes", default="", help="e.g. 256:f64,512:f32")

@@ -53,3 +53,19 @@ def test_product_arm_fails_loudly_without_a_gpu():
                           "--no-e2e"], capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert out.returncode != 0
     assert "MLUPS" not in out.stdout          # no number from any fallback
+
+
+def test_variants_cover_baseline_configs4_and_traffic_has_provenance():
+    """The default line carries short device-timed runs of the other rows of BASELINE configs[4] (>= 7 entries: D3Q15/19/27,
+    RK2, RK4, AA at 400^3 fp64, fp32 at 512^3, D3Q7 at 256^3); every ncu traffic figure names its commit and command."""
+    assert len(bench.VARIANTS) >= 7
+    got = {(n, t, p) for (n, t, p, s) in bench.VARIANTS}
+    for need in ((400, "lb_d3q15", "f64"), (400, "lb_d3q19", "f64"), (400, "lb_d3q27", "f64"), (400, "rk2", "f64"),
+                 (400, "rk4", "f64"), (512, "lb_d3q7", "f32"), (256, "lb_d3q7", "f64")):
+        assert need in got
+    assert isinstance(bench.recorded_traffic("lb_d3q7_f64_400"), int)
+    table = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    for key, entry in table.items():
+        if key.startswith("_"):
+            continue
+        assert entry["commit"] and entry["command"].startswith("ncu ") and os.path.exists(os.path.join(ROOT, entry["profile"]))

@@ -160,6 +160,23 @@ int tcp_step_end(tcp_sim *s);
  * Synchronises the stream. */
 int tcp_read_fields(tcp_sim *s, void *phi, void *u, void *p, void *T);
 
+/* The pressure read-back of tcp_read_fields for callers that must not allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): p = c_s^2 rho(phi) sum_i g~_i into `p` (HOST or
+ * DEVICE pointer, nx*ny*nz values in the simulation's precision).  tcp_read_fields stages p in a spare buffer of the
+ * workspace; this call stages it in a file-scope `static __device__` array of TCP_STATIC_SCRATCH_BYTES (8 MiB) that every
+ * GPU which loads the library holds until the process exits, and calls no cudaMalloc, cudaFree or allocating library
+ * routine.  Limit: nx*ny*nz * sizeof(real) <= TCP_STATIC_SCRATCH_BYTES, i.e. 2^20 cells in fp64 and 2^21 in fp32
+ * (BASELINE configs 1 and 2, boxes up to 101^3 / 128^3); anything larger returns TCP_EUNSUPPORTED -- use tcp_read_fields.
+ * The array is shared by every simulation and every call on that GPU and keeps the last call's contents; the kernel
+ * overwrites all of its first nx*ny*nz entries before they are copied out, so nothing has to be cleared.  The call
+ * returns after the copy has completed (it synchronises the simulation's stream), so calls made one after the other from
+ * one thread are safe; calls that overlap on the GPU (several host threads, simulations on different streams) race on the
+ * array and must be serialised by the caller.
+ * Errors: TCP_EINVAL (NULL), TCP_ESTATE (not initialised, or between tcp_step_begin and tcp_step_end),
+ * TCP_EUNSUPPORTED (box larger than the array), TCP_ECUDA. */
+#define TCP_STATIC_SCRATCH_BYTES (8u << 20)
+int tcp_read_pressure_static(tcp_sim *s, void *p);
+
 /* Wait for all work of this simulation.  Errors: TCP_ECUDA (incl. asynchronous kernel faults). */
 int tcp_synchronize(tcp_sim *s);
 

@@ -82,7 +82,7 @@ def make_params(d: dict) -> tcp_params:
 
 EXPORTS = ["tcp_params_default", "tcp_workspace_bytes", "tcp_create", "tcp_create_in", "tcp_init_fields", "tcp_set_wall_temperature",
            "tcp_set_heat_source", "tcp_step", "tcp_relax_temperature", "tcp_read_fields", "tcp_synchronize", "tcp_launch_count",
-           "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_destroy", "tcp_last_error",
+           "tcp_last_step_ms", "tcp_pattern_copy_ms", "tcp_read_pressure_static", "tcp_destroy", "tcp_last_error",
            "tcp_set_halo", "tcp_halo_phases", "tcp_halo_message_bytes", "tcp_halo_bytes", "tcp_step_begin", "tcp_step_advance",
            "tcp_step_end"]
 
@@ -110,6 +110,7 @@ def lib():
         L.tcp_step.argtypes = [vp, C.c_int]
         L.tcp_relax_temperature.argtypes = [vp, C.c_int]
         L.tcp_read_fields.argtypes = [vp, vp, vp, vp, vp]
+        L.tcp_read_pressure_static.argtypes = [vp, vp]
         L.tcp_synchronize.argtypes = [vp]
         L.tcp_launch_count.argtypes = [vp]
         L.tcp_launch_count.restype = C.c_longlong
@@ -200,6 +201,13 @@ def tcp_relax_temperature(sim, nsteps=1):
 
 def tcp_read_fields(sim, phi=None, u=None, p=None, T=None):
     _check(lib().tcp_read_fields(sim, _ptr(phi), _ptr(u), _ptr(p), _ptr(T)))
+
+
+TCP_STATIC_SCRATCH_BYTES = 8 << 20
+
+
+def tcp_read_pressure_static(sim, p):
+    _check(lib().tcp_read_pressure_static(sim, _ptr(p)))
 
 
 def tcp_synchronize(sim):

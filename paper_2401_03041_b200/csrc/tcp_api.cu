@@ -129,6 +129,13 @@ struct tcp_sim {
     cudaEvent_t ev_bnd, ev_comm;
 };
 
+// ---- tcp_read_pressure_static: scratch that no call allocates -------------------------------------------------------
+// File-scope device array (8 MiB on every GPU that loads the library, until exit).  In HOST code `g_static_scratch` is
+// only a stand-in for the symbol, not a device address: the address is resolved once per device, with that device
+// current, by cudaGetSymbolAddress in tcp_read_pressure_static, and that pointer is what the kernel gets.
+static __device__ __align__(256) unsigned char g_static_scratch[TCP_STATIC_SCRATCH_BYTES];
+static void* g_static_scratch_addr[tcp::kMaxDevices] = {};
+
 namespace {
 
 template <typename real> real* ptr(const tcp_sim* s, size_t off) { return reinterpret_cast<real*>(s->base + off); }
@@ -849,6 +856,43 @@ int tcp_step_end(tcp_sim* s) {
     if (s->phase + 1 < halo_phases(s)) return fail(TCP_ESTATE, "tcp_step_end: Runge-Kutta stages (and their transfers) are still to come, use tcp_step_advance");
     int left = 0;
     return tcp_step_advance(s, &left);
+}
+
+int tcp_read_pressure_static(tcp_sim* s, void* p) {
+    if (!s || !p) return fail(TCP_EINVAL, "NULL argument");
+    if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
+    if (s->in_step) return fail(TCP_ESTATE, "tcp_read_pressure_static between tcp_step_begin and tcp_step_end");
+    const size_t es = s->P.precision == TCP_F64 ? 8 : 4;
+    if (s->N * es > (size_t)TCP_STATIC_SCRATCH_BYTES)
+        return fail(TCP_EUNSUPPORTED, "tcp_read_pressure_static: nx*ny*nz values exceed TCP_STATIC_SCRATCH_BYTES (8 MiB: 2^20 cells in fp64, 2^21 in fp32); use tcp_read_fields");
+    DeviceScope scope(s);
+    void*& scratch = g_static_scratch_addr[s->device];
+    if (!scratch) {   // once per device, with that device current
+        void* addr = nullptr;
+        CK(cudaGetSymbolAddress(&addr, g_static_scratch));
+        scratch = addr;
+    }
+    // every entry of [0, N) is written by the kernel before the copy reads it: the last call's contents never show
+    if (s->P.precision == TCP_F64) {
+        double* out = static_cast<double*>(scratch);
+        if (s->aa_next == 1)
+            tcp::pressure_pushed_kernel<double><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(make_args<double>(s), ptr<double>(s, s->L.g[0]), ptr<double>(s, s->L.phi[s->cur]), out);
+        else
+            tcp::pressure_kernel<double><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(ptr<double>(s, s->L.g[s->cur]), ptr<double>(s, s->L.phi[s->cur]), out, (int)s->N,
+                                                                                     s->P.rho_L, s->P.rho_H - s->P.rho_L);
+    } else {
+        float* out = static_cast<float*>(scratch);
+        if (s->aa_next == 1)
+            tcp::pressure_pushed_kernel<float><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(make_args<float>(s), ptr<float>(s, s->L.g[0]), ptr<float>(s, s->L.phi[s->cur]), out);
+        else
+            tcp::pressure_kernel<float><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(ptr<float>(s, s->L.g[s->cur]), ptr<float>(s, s->L.phi[s->cur]), out, (int)s->N,
+                                                                                   (float)s->P.rho_L, (float)(s->P.rho_H - s->P.rho_L));
+    }
+    s->launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(p, scratch, s->N * es, cudaMemcpyDefault, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return TCP_OK;
 }
 
 int tcp_pattern_copy_ms(tcp_sim* s, int nlaunches, float* ms) {

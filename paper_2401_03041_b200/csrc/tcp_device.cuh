@@ -109,7 +109,7 @@ struct Nbh {
     int X[3], Y[3], Z[3];            // WALLS: coordinates of the wrapped / mirrored neighbours
     int nx, ny;
 
-    // thread id -> cell: plain x, y, z order (a z-slab visiting order was measured 2-3 % slower, profiles/r01_notes.md)
+    // thread id -> cell: plain x, y, z order (a z-slab visiting order was measured 2-3 % slower)
     template <typename real>
     __device__ __forceinline__ void init(const StepArgs<real>& A, int cell) {
         const int t = (int)fast_div((unsigned)cell, A.div_nx), x = cell - t * A.nx;

@@ -339,7 +339,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // of all NR blocks of the group that lies TCP_PF per cent of a wave ahead (NR x cells_per_block consecutive cells,
 // ~70 KB).  The HBM reads of the coming blocks are then in flight while the resident blocks are in their collision
 // phase, and their staged copies find the lines in L2: measured 12.4 -> 11.0 ms per step at 400^3 fp64 D3Q7, best at
-// half a wave, 40 % for the kernels with two blocks per SM (profiles/r01_notes.md section 15; 1.5 waves ahead the lines are evicted again before use and the step
+// half a wave, 40 % for the kernels with two blocks per SM (1.5 waves ahead the lines are evicted again before use and the step
 // slows to 14.6 ms).  A hint only: the segment is addressed without the periodic wrap and clamped into the array.
 #ifndef TCP_PF
 #define TCP_PF 50
@@ -394,7 +394,7 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
 // only g and f are staged (42 / 46 KB per block), so that three blocks fit the shared memory as for D3Q7: 400^3 D3Q15
 // 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained.  D3Q27 (15.16 -> 15.30) keeps h staged, and so does D3Q7, which
 // has its three blocks anyway: 0.5 % faster under the power cap but 4 % slower per launch at full clock (ncu 10.79 vs
-// 10.35 ms, 2 % more DRAM reads) (profiles/r01_notes.md sections 13, 26)
+// 10.35 ms, 2 % more DRAM reads)
 #ifndef TCP_HDIRECT
 #define TCP_HDIRECT 1
 #endif

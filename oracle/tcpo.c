@@ -18,13 +18,16 @@
  * Parity pins (tests/test_oracle_*.py): lattice weights (App. B), sum(phi) conservation,
  * tanh profile width, mobility decay, 1-D heat closed form, two-wall conduction, Poiseuille,
  * Laplace law, BGK reduction, layered-channel closed form (App. A), variant agreement,
- * Marangoni direction, FD operators exact on quadratics.
+ * Marangoni direction, FD operators exact on quadratics, reading S16 (tests/test_oracle_s16_rhocp.py), the
+ * 1/(rho c_p) of eq. 4, the wetting ghost rule S20 (tests/test_oracle_wetting.py: wall-normal gradient of the inclined
+ * tanh profile, sessile-droplet cap angle).
  * PARITY UNPINNED (the oracle *is* the definition): transients, the rates of
  * central moments of order >= 3 and of the trace, the lag choices S4/S10, corner ghosts on
  * domains with walls on more than one axis.
  *
  * Readings of the paper taken here are the S/G/A items of SURVEY.md 8(c), listed in DESIGN.md.
  */
+#define _USE_MATH_DEFINES
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -33,6 +36,9 @@
 #include <omp.h>
 #endif
 
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
 #define QMAX 27
 #define CS2 (1.0 / 3.0) /* lattice speed of sound squared, PAPER.md:82-86 (c_s^2), App. B */
 
@@ -59,6 +65,8 @@ typedef struct tcpo_params {
     double wall_u[3][2][3];            /* wall velocity per axis / face (moving wall; reading S18) */
     double sigma_TT;                   /* d^2 sigma / dT^2: "parabolic (or non-linear) relation between surface tension and
                                           temperature" (reading S19); 0 = the linear eq. 9 */
+    double wall_contact_angle[3][2];   /* contact angle theta in degrees of each wall [axis][face], measured inside the phi = 1 fluid
+                                          (wetting boundary condition; reading S20); 90 = neutral = mirror ghost */
     /* ---- oracle-only switches (no counterpart in the CUDA library) ---- */
     int hydro_phi_level;               /* which phi the hydrodynamic update differentiates: 0 = phi^n (reading S16, what
                                           Algorithm 1's communication order implies), 1 = phi^{n+1}
@@ -351,6 +359,10 @@ int tcpo_create(int nx, int ny, int nz, const tcpo_params *p, tcpo_sim **out) {
     if (!(p->rho_H > 0) || !(p->rho_L > 0)) return fail(TCPO_EINVAL, "rho must be > 0");
     if (!(p->kappa_H > 0) || !(p->kappa_L > 0) || !(p->cp_H > 0) || !(p->cp_L > 0))
         return fail(TCPO_EINVAL, "kappa, cp must be > 0");
+    for (int a = 0; a < 3; a++)
+        for (int fc = 0; fc < 2; fc++)
+            if (!(p->wall_contact_angle[a][fc] >= 0.0 && p->wall_contact_angle[a][fc] <= 180.0))
+                return fail(TCPO_EINVAL, "wall_contact_angle must lie in [0, 180] degrees");
     tcpo_sim *s = calloc(1, sizeof *s);
     if (!s) return fail(TCPO_ENOMEM, "calloc");
     s->nx = nx; s->ny = ny; s->nz = nz; s->N = (size_t)nx * ny * nz; s->P = *p;
@@ -458,9 +470,32 @@ static nbr neighbour(const tcpo_sim *s, int x, int y, int z, int dx, int dy, int
     return r;
 }
 
-/* phi at a neighbour: ghost = mirror cell (neutral wetting) */
+/* Wetting boundary condition (PAPER.md:307 names it -- "based on that proposed by Fakhari et al. [34]" -- and prints no
+ * formula; reading S20).  At a wall with unit normal n_w pointing into the fluid the equilibrium profile
+ * phi = 1/2 [1 + tanh(2 s / xi)] (eq. 35) that meets the wall at the contact angle theta (measured inside the
+ * phi = 1 fluid) satisfies
+ *     n_w . grad phi = Theta phi_w (1 - phi_w),      Theta = -(4 / xi) cos(theta)
+ * (|grad phi| = (4/xi) phi (1 - phi) on that profile, and the interface normal grad phi / |grad phi| makes the angle
+ * pi - theta with n_w).  With the wall half a cell outside the first fluid cell (S9): phi_w = (phi_f + phi_g) / 2 and
+ * n_w . grad phi = (phi_f - phi_g) / 1, phi_f the fluid cell across the wall from the ghost cell.  Eliminating phi_g:
+ *     a phi_w^2 - (1 + a) phi_w + phi_f = 0,   a = Theta / 2,
+ * of which the root that tends to phi_f for a -> 0 is taken, and phi_g = 2 phi_w - phi_f.  theta = 90 degrees: a = 0,
+ * phi_g = phi_f, the mirror ghost of S9.  The quadratic is solved the textbook cancellation-free way
+ * (q = -(B + sgn(B) sqrt(B^2 - 4AC)) / 2, roots q / A and C / q; here B = -(1 + a) < 0 and the wanted root is C / q). */
+static double wetting_ghost(const tcpo_sim *s, int axis, int face, double phi_f) {
+    double theta = s->P.wall_contact_angle[axis][face];
+    if (theta == 90.0) return phi_f;
+    double a = 0.5 * (-(4.0 / s->P.xi) * cos(theta * M_PI / 180.0));
+    double A = a, B = -(1.0 + a), C = phi_f;
+    double q = -0.5 * (B - sqrt(B * B - 4.0 * A * C));
+    double phi_w = C / q;
+    return 2.0 * phi_w - phi_f;
+}
+
+/* phi at a neighbour: ghost from the mirror cell by the wetting condition (neutral wetting: the mirror cell's value) */
 static double phi_at(const tcpo_sim *s, const double *phi, int x, int y, int z, int dx, int dy, int dz) {
     nbr r = neighbour(s, x, y, z, dx, dy, dz);
+    if (r.axis >= 0) return wetting_ghost(s, r.axis, r.face, phi[r.idx]);
     return phi[r.idx];
 }
 

@@ -64,10 +64,16 @@ typedef struct tcp_params {
                                           + sigma_TT (T - T_ref)^2 / 2 (self-rewetting fluids); the
                                           Marangoni term of eq. 8 then carries d sigma/dT = sigma_T + sigma_TT (T - T_ref).
                                           Default 0 = eq. 9 as printed */
+    double wall_contact_angle[3][2];   /* wetting boundary condition (refs. [34], [35]): contact angle of each wall
+                                          [axis][face] in degrees, 0..180, measured inside the phi = 1 fluid.  The ghost value of
+                                          phi behind the wall follows from n_w . grad phi = -(4 / xi) cos(theta) phi_w (1 - phi_w)
+                                          with phi_w = (phi_f + phi_g) / 2 at the wall half a cell outside the first cell:
+                                          a phi_w^2 - (1 + a) phi_w + phi_f = 0, a = -(2 / xi) cos(theta), phi_g = 2 phi_w - phi_f.
+                                          Default 90 = neutral wetting = mirror ghost */
 } tcp_params;
 
 /* Fill *p with the defaults: struct_size, fp64, thermal LB D3Q7, two-grid, periodic x 3, rho = 1, tau = 0.6, xi = 4,
- * M = 0.05, sigma = 0, kappa = 0.2, c_p = 1, no gravity, walls at rest and at T = 0, s_bulk = s_high = 1 (the closed-form
+ * M = 0.05, sigma = 0, kappa = 0.2, c_p = 1, no gravity, walls at rest, at T = 0 and neutrally wetting (90 degrees), s_bulk = s_high = 1 (the closed-form
  * central-moment collision), eps_normal = 1e-32.  A zero-initialised struct is NOT valid (eps_normal = 0 makes the
  * interface normal 0/0 in the bulk, s_bulk = s_high = 0 are not relaxation rates): tcp_create rejects it with TCP_EINVAL.
  * Errors: TCP_EINVAL (p NULL). */

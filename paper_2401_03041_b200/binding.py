@@ -37,6 +37,7 @@ class tcp_params(C.Structure):
         ("eps_normal", C.c_double),
         ("wall_u", ((C.c_double * 3) * 2) * 3),
         ("sigma_TT", C.c_double),
+        ("wall_contact_angle", (C.c_double * 2) * 3),
     ]
 
 
@@ -49,6 +50,7 @@ PARAM_DEFAULTS = dict(
     s_bulk=1.0, s_high=1.0, high_rate_equals_shear=0, eps_normal=1e-32,
     wall_u=(((0.0,) * 3,) * 2,) * 3,
     sigma_TT=0.0,
+    wall_contact_angle=((90.0, 90.0), (90.0, 90.0), (90.0, 90.0)),
 )
 
 
@@ -69,6 +71,7 @@ def make_params(d: dict) -> tcp_params:
         p.gravity[a] = float(v["gravity"][a])
         for f in range(2):
             p.wall_T[a][f] = float(v["wall_T"][a][f])
+            p.wall_contact_angle[a][f] = float(v["wall_contact_angle"][a][f])
     for k in ("rho_H", "rho_L", "tau_H", "tau_L", "xi", "M", "sigma_ref", "sigma_T", "sigma_TT", "T_ref",
               "kappa_H", "kappa_L", "cp_H", "cp_L", "s_bulk", "s_high", "eps_normal"):
         setattr(p, k, float(v[k]))

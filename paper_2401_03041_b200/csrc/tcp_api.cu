@@ -71,6 +71,10 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
     // zero-initialises the struct gets an error, not NaNs; tcp_params_default() fills the documented defaults
     if (!(p->eps_normal > 0)) return fail(TCP_EINVAL, "eps_normal must be > 0 (default 1e-32, see tcp_params_default)");
     if (!(p->s_bulk > 0 && p->s_bulk < 2) || !(p->s_high > 0 && p->s_high < 2)) return fail(TCP_EINVAL, "s_bulk and s_high must lie in (0, 2) (default 1, see tcp_params_default)");
+    for (int a = 0; a < 3; ++a)
+        for (int fc = 0; fc < 2; ++fc)
+            if (!(p->wall_contact_angle[a][fc] >= 0.0 && p->wall_contact_angle[a][fc] <= 180.0))
+                return fail(TCP_EINVAL, "wall_contact_angle must lie in [0, 180] degrees (default 90, see tcp_params_default)");
     if (p->high_rate_equals_shear != 0 && p->high_rate_equals_shear != 1) return fail(TCP_EINVAL, "high_rate_equals_shear must be 0 or 1");
     return TCP_OK;
 }
@@ -199,6 +203,15 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
                 A.wall_u[a][fc][k] = (real)P.wall_u[a][fc][k];
                 if (P.wall_u[a][fc][k] != 0.0) A.moving = 1;
             }
+    // wetting (reading S20): a = -(2 / xi) cos(theta) per wall; exactly 0 for the neutral 90 degrees
+    A.wetting = 0;
+    for (int a = 0; a < 3; ++a)
+        for (int fc = 0; fc < 2; ++fc) {
+            const double th = P.wall_contact_angle[a][fc];
+            const double wa = (th == 90.0 || P.bc[a] != TCP_BC_WALLS) ? 0.0 : -(2.0 / P.xi) * std::cos(th * 3.14159265358979323846 / 180.0);
+            A.wet_a[a][fc] = (real)wa;
+            if (wa != 0.0) A.wetting = 1;
+        }
     // S8: eps keeps n = grad phi / |grad phi| finite where grad phi vanishes.  In fp32 a gradient
     // below ~1e-6 is round-off of phi ~ 1, and a round-off-directed sharpening flux makes phi = 0 / 1
     // unstable to noise (measured: 1e-4 error after 100 steps next to a wall), so eps is floored there.
@@ -693,6 +706,7 @@ int tcp_params_default(tcp_params* p) {
     p->cp_H = p->cp_L = 1.0;
     p->s_bulk = p->s_high = 1.0;
     p->eps_normal = 1e-32;
+    for (int a = 0; a < 3; ++a) p->wall_contact_angle[a][0] = p->wall_contact_angle[a][1] = 90.0;
     return TCP_OK;
 }
 

@@ -40,6 +40,8 @@ struct StepArgs {
     real s_bulk, s_high, eps;
     int moving;                      // any wall velocity non-zero
     real wall_u[3][2][3];            // wall velocity [axis][face][component] (moving wall, reading S18)
+    int wetting;                     // any wall with a contact angle other than 90 degrees
+    real wet_a[3][2];                // a = -(2 / xi) cos(theta) of each wall (wetting boundary condition, reading S20); 0 = neutral
 };
 
 // packed pairs: the arrays are plain float arrays, the scalars are broadcast pairs
@@ -71,18 +73,21 @@ struct StepArgs<f32x2> {
     f32x2 s_bulk, s_high, eps;
     int moving;
     float wall_u[3][2][3];
+    int wetting;
+    float wet_a[3][2];
     __host__ explicit StepArgs(const StepArgs<float>& A)
         : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), cell0(A.cell0), cell1(A.cell1), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
           f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src), rk1_out(A.rk1_out), rk1_acc(A.rk1_acc), rk1_c_out(A.rk1_c_out), rk1_c_acc(A.rk1_c_acc),
           rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), inv_xi(A.inv_xi), sigma_ref(A.sigma_ref),
           sigma_T(A.sigma_T), T_ref(A.T_ref), sigma_TT(A.sigma_TT), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
-          s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving) {
+          s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving), wetting(A.wetting) {
         for (int k = 0; k < 3; ++k) { div_nx[k] = A.div_nx[k]; div_ny[k] = A.div_ny[k]; div_hx[k] = A.div_hx[k]; }
         for (int a = 0; a < 3; ++a) {
             wall[a] = A.wall[a];
             grav[a] = f32x2(A.grav[a]);
             for (int f = 0; f < 2; ++f) {
                 wallT[a][f] = A.wallT[a][f];
+                wet_a[a][f] = A.wet_a[a][f];
                 for (int k = 0; k < 3; ++k) wall_u[a][f][k] = A.wall_u[a][f][k];
             }
         }
@@ -179,6 +184,18 @@ __device__ __forceinline__ real wall_velocity_term(const StepArgs<real>& A, cons
     return real(6.0 * weight(27, cls27(q27i))) * (real(cx) * U[0] + real(cy) * U[1] + real(cz) * U[2]);
 }
 
+// Wetting boundary condition (refs. [34], [35]; reading S20): ghost value of phi behind a wall with
+// a = -(2 / xi) cos(theta), from the fluid cell phi_f across the wall:  n_w . grad phi = -(4 / xi) cos(theta) phi_w (1 - phi_w)
+// with phi_w = (phi_f + phi_g) / 2 gives  a phi_w^2 - (1 + a) phi_w + phi_f = 0; the root that tends to phi_f for a -> 0,
+// written without cancellation: phi_w = 2 phi_f / ((1 + a) + sqrt((1 + a)^2 - 4 a phi_f));  phi_g = 2 phi_w - phi_f.
+// a = 0 returns phi_f exactly (the mirror ghost of S9).
+template <typename scalar>
+__device__ __forceinline__ scalar wetting_ghost(scalar a, scalar phi_f) {
+    const scalar b = scalar(1) + a;
+    const scalar phi_w = (scalar(2) * phi_f) / (b + sqrt(b * b - scalar(4) * a * phi_f));
+    return scalar(2) * phi_w - phi_f;
+}
+
 // ---------------------------------------------------------------------------------------------
 // isotropic finite differences with the D3Q27 weights (reading S3), evaluated as a tensor product:
 //   grad_x = D_x S_y S_z,  lap = 6 (S_x S_y S_z - 1),   S = [1/6, 2/3, 1/6],  D = [-1/2, 0, 1/2]
@@ -205,6 +222,11 @@ __device__ __forceinline__ void stencil27(const StepArgs<real>& A, const Nbh<WAL
                     int face = 0;
                     const int ax = nb.crossed(ox, oy, oz, face);
                     if (ax >= 0) t = real(2) * wall_temperature(A, nb, ax, face, ox, oy, oz) - t;
+                }
+                if (WALLS && !IS_TEMP && A.wetting) {   // t is the mirror cell's value: first crossed wall in x, y, z order (S17)
+                    int face = 0;
+                    const int ax = nb.crossed(ox, oy, oz, face);
+                    if (ax >= 0) t = wetting_ghost<real>(A.wet_a[ax][face], t);
                 }
                 v[ox + 1] = t;
             }

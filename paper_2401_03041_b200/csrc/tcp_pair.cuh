@@ -110,6 +110,15 @@ __device__ __forceinline__ void stencil27_pair(const StepArgs<f32x2>& A, const N
                     v0 = 2.0f * wl.v.x - v0; v1 = 2.0f * wl.v.y - v1; v2 = 2.0f * wr.v.x - v2; v3 = 2.0f * wr.v.y - v3;
                 }
             }
+            if (WALLS && !IS_TEMP && A.wetting) {   // wetting ghost row (reading S20); the row's four values are mirror cells
+                int face = 0;
+                const int ax = nb.crossed(oy, oz, face);
+                if (ax >= 0) {
+                    const float a = A.wet_a[ax][face];
+                    v0 = wetting_ghost<float>(a, v0); v1 = wetting_ghost<float>(a, v1);
+                    v2 = wetting_ghost<float>(a, v2); v3 = wetting_ghost<float>(a, v3);
+                }
+            }
             const f32x2 m(v0, v1), c(v1, v2), p(v2, v3);
             if (oy == 0 && oz == 0) centre = c;
             sx[oy + 1] = (m + p) + four * c;

@@ -86,7 +86,15 @@ __global__ void __launch_bounds__(kRkTX * kRkTY, rk_min_blocks<real, HAS_DK>()) 
             if (!e_on[i]) continue;
             const int idx = e_idx2d[i] + sz * Z;
             real vy = __ldg(R.Y + idx);
-            if (HAS_DK) pfP[i] = __ldg(A.phi_in + idx);
+            if (HAS_DK) {
+                real vp = __ldg(A.phi_in + idx);
+                if (WALLS && A.wetting) {   // wetting ghost (reading S20): first crossed wall in x, y, z order, as in stencil27
+                    if (e_fx[i] >= 0) vp = wetting_ghost<real>(A.wet_a[0][e_fx[i]], vp);
+                    else if (e_fy[i] >= 0) vp = wetting_ghost<real>(A.wet_a[1][e_fy[i]], vp);
+                    else if (fz >= 0) vp = wetting_ghost<real>(A.wet_a[2][fz], vp);
+                }
+                pfP[i] = vp;
+            }
             if (WALLS) {   // Dirichlet ghost 2 T_w - Y(mirror); first crossed axis in x, y, z order (S9, S17)
                 if (e_fx[i] >= 0) vy = real(2) * A.wallT[0][e_fx[i]][Z * A.ny + e_tang_y[i]] - vy;
                 else if (e_fy[i] >= 0) vy = real(2) * A.wallT[1][e_fy[i]][Z * A.nx + e_tang_x[i]] - vy;

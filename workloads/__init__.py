@@ -10,8 +10,8 @@ DESIGN.md.
 All arrays are torch float64 tensors laid out [nz][ny][nx] (x fastest); u0 is [3][nz][ny][nx].
 """
 from .configs import (Workload, static_droplet, layered_channel, droplet_in_gradient,
-                      thermal_tweezer, perf_box, laser_source, BENCH_FLUID)
+                      thermal_tweezer, perf_box, laser_source, laser_channel, BENCH_FLUID)
 from .analytic import layered_channel_closed_form
 
 __all__ = ["Workload", "static_droplet", "layered_channel", "droplet_in_gradient",
-           "thermal_tweezer", "perf_box", "laser_source", "BENCH_FLUID", "layered_channel_closed_form"]
+           "thermal_tweezer", "perf_box", "laser_source", "laser_channel", "BENCH_FLUID", "layered_channel_closed_form"]

@@ -67,6 +67,8 @@ typedef struct tcpo_params {
                                           temperature" (reading S19); 0 = the linear eq. 9 */
     double wall_contact_angle[3][2];   /* contact angle theta in degrees of each wall [axis][face], measured inside the phi = 1 fluid
                                           (wetting boundary condition; reading S20); 90 = neutral = mirror ghost */
+    int hydro_lattice;                 /* 27 (default) or 19: lattice of the hydrodynamic populations g ("hydrodynamic LBM solvers
+                                          often rely on a D3Q19 or D3Q27 stencil"); weights App. B.3, basis S2 */
     /* ---- oracle-only switches (no counterpart in the CUDA library) ---- */
     int hydro_phi_level;               /* which phi the hydrodynamic update differentiates: 0 = phi^n (reading S16, what
                                           Algorithm 1's communication order implies), 1 = phi^{n+1}
@@ -297,7 +299,7 @@ typedef struct tcpo_sim {
     int nx, ny, nz;
     size_t N;
     tcpo_params P;
-    lattice L27, LT; /* D3Q27 for h, g and the FD stencils; LT for f */
+    lattice L27, LT, LH; /* D3Q27 for h and the FD stencils; LT for f; LH (D3Q27 or D3Q19) for g */
     int thermal_is_lb;
     double *h, *h2, *g, *g2, *f, *f2; /* post-collision populations [Q][N], two grids */
     double *phi, *phi2, *T, *T2, *u;  /* u = [3][N] */
@@ -354,6 +356,7 @@ int tcpo_create(int nx, int ny, int nz, const tcpo_params *p, tcpo_sim **out) {
         if (p->bc[a] == TCPO_WALLS && n[a] < 2) return fail(TCPO_EINVAL, "wall axis needs n >= 2");
     }
     if (p->thermal < TCPO_LB_D3Q7 || p->thermal > TCPO_RK4) return fail(TCPO_EINVAL, "bad thermal variant");
+    if (p->hydro_lattice != 27 && p->hydro_lattice != 19) return fail(TCPO_EINVAL, "hydro_lattice must be 27 or 19");
     if (!(p->tau_H > -0.5) || !(p->tau_L > -0.5)) return fail(TCPO_EINVAL, "tau <= -1/2");
     if (!(p->M > 0) || !(p->xi > 0)) return fail(TCPO_EINVAL, "M, xi must be > 0");
     if (!(p->rho_H > 0) || !(p->rho_L > 0)) return fail(TCPO_EINVAL, "rho must be > 0");
@@ -367,12 +370,13 @@ int tcpo_create(int nx, int ny, int nz, const tcpo_params *p, tcpo_sim **out) {
     if (!s) return fail(TCPO_ENOMEM, "calloc");
     s->nx = nx; s->ny = ny; s->nz = nz; s->N = (size_t)nx * ny * nz; s->P = *p;
     lattice_build(&s->L27, 27);
+    lattice_build(&s->LH, p->hydro_lattice);
     static const int QT[4] = {7, 15, 19, 27};
     s->thermal_is_lb = p->thermal <= TCPO_LB_D3Q27;
     lattice_build(&s->LT, s->thermal_is_lb ? QT[p->thermal] : 7);
     size_t N = s->N;
     s->h = calloc(27 * N, 8); s->h2 = calloc(27 * N, 8);
-    s->g = calloc(27 * N, 8); s->g2 = calloc(27 * N, 8);
+    s->g = calloc((size_t)p->hydro_lattice * N, 8); s->g2 = calloc((size_t)p->hydro_lattice * N, 8);
     s->phi = calloc(N, 8); s->phi2 = calloc(N, 8);
     s->T = calloc(N, 8); s->T2 = calloc(N, 8); s->u = calloc(3 * N, 8);
     int ok = s->h && s->h2 && s->g && s->g2 && s->phi && s->phi2 && s->T && s->T2 && s->u;
@@ -425,8 +429,8 @@ int tcpo_init_fields(tcpo_sim *s, const double *phi, const double *u, const doub
         double e[QMAX];
         eq_scalar(&s->L27, s->phi[k], uu, e);
         for (int i = 0; i < 27; i++) s->h[i * N + k] = e[i];
-        eq_hydro(&s->L27, 0.0, uu, e);
-        for (int i = 0; i < 27; i++) s->g[i * N + k] = e[i];
+        eq_hydro(&s->LH, 0.0, uu, e);
+        for (int i = 0; i < s->LH.Q; i++) s->g[i * N + k] = e[i];
         if (s->thermal_is_lb) {
             eq_scalar(&s->LT, s->T[k], uu, e);
             for (int i = 0; i < s->LT.Q; i++) s->f[i * N + k] = e[i];
@@ -600,7 +604,7 @@ static int update_h(tcpo_sim *s) {
 
 /* O4-O7: hydrodynamic LB (eqs. 16-22 and 7-9) */
 static int update_g(tcpo_sim *s) {
-    const lattice *L = &s->L27;
+    const lattice *L = &s->LH;  /* D3Q27 or D3Q19 */
     const tcpo_params *P = &s->P;
     size_t N = s->N;
     int bad = 0;
@@ -612,7 +616,7 @@ static int update_g(tcpo_sim *s) {
                 size_t k = (size_t)x + (size_t)s->nx * ((size_t)y + (size_t)s->ny * z);
                 double gp[QMAX], geq[QMAX], gout[QMAX];
                 double pstar = 0.0, j[3] = {0, 0, 0};
-                for (int i = 0; i < 27; i++) { /* O4, eq. 17 */
+                for (int i = 0; i < L->Q; i++) { /* O4, eq. 17 */
                     gp[i] = pull_bb_moving(s, L, s->g, i, x, y, z, k);
                     pstar += gp[i];
                     for (int al = 0; al < 3; al++) j[al] += L->c[i][al] * gp[i];
@@ -645,7 +649,7 @@ static int update_g(tcpo_sim *s) {
                 /* non-equilibrium second moments about g_eq(p*, u*) and eq. 21 */
                 eq_hydro(L, pstar, ustar, geq);
                 double Pi[3][3] = {{0}};
-                for (int i = 0; i < 27; i++)
+                for (int i = 0; i < L->Q; i++)
                     for (int al = 0; al < 3; al++)
                         for (int be = 0; be < 3; be++) Pi[al][be] += L->c[i][al] * L->c[i][be] * (gp[i] - geq[i]);
                 for (int al = 0; al < 3; al++) {
@@ -661,7 +665,7 @@ static int update_g(tcpo_sim *s) {
                 rates R = {1.0, 1.0, om, P->s_bulk, P->s_high};
                 if (P->high_rate_equals_shear) { R.r0 = R.r1 = R.r2s = R.r2b = R.r3 = om; }
                 if (collide_generic(L, &R, u, gp, geq, a, gout)) bad |= 1;
-                for (int i = 0; i < 27; i++) s->g2[(size_t)i * N + k] = gout[i];
+                for (int i = 0; i < L->Q; i++) s->g2[(size_t)i * N + k] = gout[i];
                 s->u[k] = u[0]; s->u[N + k] = u[1]; s->u[2 * N + k] = u[2]; /* u is only read locally */
             }
     if (bad) return fail(TCPO_ESTATE, "singular K in update_g");
@@ -790,7 +794,7 @@ int tcpo_read_fields(tcpo_sim *s, double *phi, double *u, double *p, double *T) 
     if (p)
         for (size_t k = 0; k < N; k++) {
             double ps = 0.0;
-            for (int i = 0; i < 27; i++) ps += s->g[(size_t)i * N + k];
+            for (int i = 0; i < s->LH.Q; i++) ps += s->g[(size_t)i * N + k];
             p[k] = CS2 * lerp_phi(s->P.rho_L, s->P.rho_H, s->phi[k]) * ps;
         }
     return TCPO_OK;
@@ -803,7 +807,7 @@ int tcpo_read_fields(tcpo_sim *s, double *phi, double *u, double *p, double *T) 
 int tcpo_read_populations(tcpo_sim *s, int which, double *out) {
     if (!s || !out) return fail(TCPO_EINVAL, "null");
     const double *src = which == 0 ? s->h : (which == 1 ? s->g : s->f);
-    int Q = which == 2 ? s->LT.Q : 27;
+    int Q = which == 2 ? s->LT.Q : (which == 1 ? s->LH.Q : 27);
     if (!src) return fail(TCPO_ESTATE, "no such populations");
     memcpy(out, src, (size_t)Q * s->N * 8);
     return TCPO_OK;

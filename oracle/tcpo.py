@@ -33,6 +33,7 @@ class Params(C.Structure):
         ("wall_u", ((C.c_double * 3) * 2) * 3),
         ("sigma_TT", C.c_double),
         ("wall_contact_angle", (C.c_double * 2) * 3),   # degrees, reading S20
+        ("hydro_lattice", C.c_int),        # 27 or 19
         ("hydro_phi_level", C.c_int),      # oracle-only (reading S16): 0 = phi^n, 1 = phi^{n+1}
     ]
 
@@ -47,6 +48,7 @@ DEFAULTS = dict(
     wall_u=(((0.0,) * 3,) * 2,) * 3,
     sigma_TT=0.0,
     wall_contact_angle=((90.0, 90.0), (90.0, 90.0), (90.0, 90.0)),
+    hydro_lattice=27,
     hydro_phi_level=0,
 )
 
@@ -75,6 +77,7 @@ def make_params(d: dict) -> Params:
         setattr(p, k, float(v[k]))
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
     p.hydro_phi_level = int(v["hydro_phi_level"])
+    p.hydro_lattice = int(v["hydro_lattice"])
     for a in range(3):
         for f in range(2):
             for c in range(3):
@@ -199,7 +202,7 @@ class Oracle:
         return phi, u, p, T
 
     def read_populations(self, which):
-        q = 27 if which in (0, 1) else self.q_thermal
+        q = 27 if which == 0 else (self._p.hydro_lattice if which == 1 else self.q_thermal)
         out = np.empty((q,) + self.shape)
         _check(lib().tcpo_read_populations(self._h, which, _dp(out)))
         return out

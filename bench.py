@@ -36,19 +36,19 @@ METRIC = "MLUPS of full coupled step on 1 B200; % of HBM roofline (bytes/cell)"
 QT = {"lb_d3q7": 7, "lb_d3q15": 15, "lb_d3q19": 19, "lb_d3q27": 27, "rk2": 0, "rk4": 0}
 
 
-def fused_kernel_values_per_cell(thermal):
+def fused_kernel_values_per_cell(thermal, hydro=27):
     """Algorithmic values moved per cell by the dominant kernel: h, g read +
-    written (54 + 54), f read + written (2 Q_T), phi read + written (2), T read (+ written on the LB
+    written (54 + 2 Q_H), f read + written (2 Q_T), phi read + written (2), T read (+ written on the LB
     path), u read + written (6)."""
     q = QT[thermal]
-    return 54 + 54 + 2 * q + 2 + (2 if q else 1) + 6
+    return 54 + 2 * hydro + 2 * q + 2 + (2 if q else 1) + 6
 
 
-def step_values_per_cell(thermal):
+def step_values_per_cell(thermal, hydro=27):
     """Whole step.  The benchmark fluid has kappa_H = kappa_L, so the first Runge-Kutta stage runs inside the fused
     kernel and costs only its stores (Y1, and the RK4 accumulator); the stages that remain are
     kernels of their own: read Y, phi, u(3), Tn (+ accumulator), write out (+ accumulator)."""
-    v = fused_kernel_values_per_cell(thermal)
+    v = fused_kernel_values_per_cell(thermal, hydro)
     if thermal == "rk2":
         v += 1 + 7
     if thermal == "rk4":
@@ -176,13 +176,13 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def timed_variant(tcp, n, thermal, prec, streaming, warmup, steps, device_index, peak):
+def timed_variant(tcp, n, thermal, prec, streaming, warmup, steps, device_index, peak, hydro=27):
     """One short device-timed run of another row of BASELINE configs[4] (W >= 3 warm-up steps, K >= 20 timed, CUDA
     events of the library around its own launches, clocks sampled during the timed region)."""
     es = 8 if prec == "f64" else 4
     tdt = torch.float64 if prec == "f64" else torch.float32
     wl = W.perf_box(n, thermal=thermal, device="cuda")
-    sim = tcp.Simulation(n, n, n, dict(wl.params, precision=prec, streaming=streaming))
+    sim = tcp.Simulation(n, n, n, dict(wl.params, precision=prec, streaming=streaming, hydro_lattice=hydro))
     sim.init_fields(wl.phi.to(tdt).contiguous(), None, wl.T.to(tdt).contiguous())
     del wl
     sim.step(max(warmup, 3))
@@ -198,9 +198,9 @@ def timed_variant(tcp, n, thermal, prec, streaming, warmup, steps, device_index,
     sim.close()
     del sim
     torch.cuda.empty_cache()
-    bpc = step_values_per_cell(thermal) * es
+    bpc = step_values_per_cell(thermal, hydro) * es
     gbs = bpc * n ** 3 / (ms * 1e-3) / 1e9
-    return {"workload": f"perf_box {n}^3", "thermal": thermal, "dtype": prec, "streaming": streaming, "steps": steps,
+    return {"workload": f"perf_box {n}^3", "thermal": thermal, "hydro": f"D3Q{hydro}", "dtype": prec, "streaming": streaming, "steps": steps,
             "warmup": max(warmup, 3), "ms_per_step": ms, "mlups": n ** 3 / (ms * 1e-3) / 1e6, "step_bytes_per_cell": bpc,
             "achieved_gbs": gbs, "frac": gbs / peak, "frac_of_nominal": gbs / NOMINAL_HBM_GBS, "gpu_launches": launches,
             "clocks": clocks, "finite": finite}
@@ -208,7 +208,8 @@ def timed_variant(tcp, n, thermal, prec, streaming, warmup, steps, device_index,
 
 VARIANTS = [(400, "lb_d3q15", "f64", "two_grid"), (400, "lb_d3q19", "f64", "two_grid"), (400, "lb_d3q27", "f64", "two_grid"),
             (400, "rk2", "f64", "two_grid"), (400, "rk4", "f64", "two_grid"), (400, "lb_d3q7", "f64", "aa"),
-            (512, "lb_d3q7", "f32", "two_grid"), (512, "rk2", "f32", "two_grid"), (256, "lb_d3q7", "f64", "two_grid")]
+            (512, "lb_d3q7", "f32", "two_grid"), (512, "rk2", "f32", "two_grid"), (256, "lb_d3q7", "f64", "two_grid"),
+            (400, "lb_d3q7", "f64", "two_grid", 19)]          # last entry: D3Q19 hydrodynamic lattice (928 B per cell)
 
 
 def run_ours(args):
@@ -229,7 +230,7 @@ def run_ours(args):
     tdt = torch.float64 if prec == "f64" else torch.float32
     wl = W.perf_box(n, thermal=thermal, device="cuda", seed=20240103 + n + rank)
     N = wl.cells
-    params = dict(wl.params, precision=prec, streaming=args.streaming)
+    params = dict(wl.params, precision=prec, streaming=args.streaming, hydro_lattice=args.hydro)
     sim = tcp.Simulation(n, n, n, params)
     phi_d, T_d = wl.phi.to(tdt).contiguous(), wl.T.to(tdt).contiguous()
     wl_notes, wl_fields = wl.notes, (wl.phi, wl.T)
@@ -315,8 +316,8 @@ def run_ours(args):
         return
 
     peak, peak_src = hbm_peak()
-    fused_bytes = fused_kernel_values_per_cell(thermal) * es * N
-    step_bytes = step_values_per_cell(thermal) * es * N
+    fused_bytes = fused_kernel_values_per_cell(thermal, args.hydro) * es * N
+    step_bytes = step_values_per_cell(thermal, args.hydro) * es * N
     if QT[thermal]:
         k_ms = kernel_ms / args.steps                      # one fused kernel per step
         achieved = fused_bytes / (k_ms * 1e-3) / 1e9
@@ -326,7 +327,7 @@ def run_ours(args):
         achieved = step_bytes / (k_ms * 1e-3) / 1e9        # whole step (fused kernel + RK stages)
         kname = "fused_step_async_kernel + rk_stage_march_kernel (whole step)"
     alg_bytes = fused_bytes if QT[thermal] else step_bytes
-    tkey = f"{thermal}_{prec}_{n}" + ("_aa" if args.streaming == "aa" else "")
+    tkey = f"{thermal}_{prec}_{n}" + ("_aa" if args.streaming == "aa" else "") + ("_q19" if args.hydro == 19 else "")
     if sustained is not None:
         sus_gbs = alg_bytes / (sustained["ms_per_step"] * 1e-3) / 1e9
         sustained.update({"achieved": sus_gbs, "frac": sus_gbs / peak, "frac_of_nominal": sus_gbs / NOMINAL_HBM_GBS})
@@ -342,9 +343,9 @@ def run_ours(args):
                 "pattern_copy": None if pattern_ms is None else {"ms": pattern_ms, "gbs": fused_bytes / (pattern_ms * 1e-3) / 1e9,
                                                                   "frac_of_peak": fused_bytes / (pattern_ms * 1e-3) / 1e9 / peak}}
     variants = None
-    if world == 1 and not args.no_variants and (n, thermal, prec, args.streaming) == (400, "lb_d3q7", "f64", "two_grid"):
+    if world == 1 and not args.no_variants and (n, thermal, prec, args.streaming, args.hydro) == (400, "lb_d3q7", "f64", "two_grid", 27):
         # the other rows of BASELINE configs[4] under the same clock (the headline above stays the metric's line)
-        variants = [timed_variant(tcp, *v, args.warmup, max(args.variant_steps, 20), local, peak) for v in VARIANTS]
+        variants = [timed_variant(tcp, *v[:4], args.warmup, max(args.variant_steps, 20), local, peak, *v[4:]) for v in VARIANTS]
     cpu = None
     if not args.no_cpu:
         v, _, cores, sample = oracle_throughput(thermal)
@@ -353,7 +354,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": prec, "data": "synthetic",
-            "config": {"workload": f"perf_box {n}^3 periodic (BASELINE configs[4]), hydro D3Q27 CM, phase D3Q27, thermal {thermal}, streaming {args.streaming}",
+            "config": {"workload": f"perf_box {n}^3 periodic (BASELINE configs[4]), hydro D3Q{args.hydro} CM, phase D3Q27, thermal {thermal}, streaming {args.streaming}",
                        "cells_per_gpu": N, "parallelism": "replicas" if world > 1 else "single GPU",
                        "l2": f"working set {step_bytes / 1e9:.1f} GB per step >> 126 MB L2, no flush needed",
                        "e2e_steps": args.steps, "notes": wl_notes},
@@ -467,6 +468,7 @@ def main():
     ap.add_argument("--thermal", default="lb_d3q7", choices=sorted(QT))
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--streaming", default="two_grid", choices=["two_grid", "aa"])
+    ap.add_argument("--hydro", type=int, default=27, choices=[27, 19], help="hydrodynamic lattice (BASELINE's metric is quoted on D3Q27)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-size", type=int, default=64)
     ap.add_argument("--no-e2e", action="store_true")

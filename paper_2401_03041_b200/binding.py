@@ -38,6 +38,7 @@ class tcp_params(C.Structure):
         ("wall_u", ((C.c_double * 3) * 2) * 3),
         ("sigma_TT", C.c_double),
         ("wall_contact_angle", (C.c_double * 2) * 3),
+        ("hydro_lattice", C.c_int),
     ]
 
 
@@ -51,6 +52,7 @@ PARAM_DEFAULTS = dict(
     wall_u=(((0.0,) * 3,) * 2,) * 3,
     sigma_TT=0.0,
     wall_contact_angle=((90.0, 90.0), (90.0, 90.0), (90.0, 90.0)),
+    hydro_lattice=27,
 )
 
 
@@ -76,6 +78,7 @@ def make_params(d: dict) -> tcp_params:
               "kappa_H", "kappa_L", "cp_H", "cp_L", "s_bulk", "s_high", "eps_normal"):
         setattr(p, k, float(v[k]))
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
+    p.hydro_lattice = int(v["hydro_lattice"])
     for a in range(3):
         for f in range(2):
             for c in range(3):

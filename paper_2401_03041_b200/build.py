@@ -1,7 +1,7 @@
 """Build libtcp.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
 
 The fused step kernels are ~70 template instantiations; they live in four translation units
-(precision x boundary kind) that are compiled in parallel and linked with the host API.
+(precision x boundary kind x hydrodynamic lattice) that are compiled in parallel and linked with the host API.
 
 Usage: python -m paper_2401_03041_b200.build [--force] [--verbose]
 """
@@ -14,7 +14,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtcp.so")
 SOURCES = ["tcp_api.cu", "tcp_fused_f64_periodic.cu", "tcp_fused_f64_walls.cu", "tcp_fused_f32_periodic.cu",
-           "tcp_fused_f32_walls.cu"]
+           "tcp_fused_f32_walls.cu", "tcp_fused_f64_periodic_q19.cu", "tcp_fused_f64_walls_q19.cu",
+           "tcp_fused_f32_periodic_q19.cu", "tcp_fused_f32_walls_q19.cu"]
 HEADERS = ["tcp_lattice.cuh", "tcp_device.cuh", "tcp_kernels.cuh", "tcp_step.cuh", "tcp_rk.cuh",
            "tcp_launch.h", "tcp_launch.inl", "tcp_real.cuh", "tcp_pair.cuh", "tcp_halo.cuh"]
 # IEEE division / sqrt kept (no fast-math); FMA contraction on

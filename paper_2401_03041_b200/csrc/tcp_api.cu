@@ -75,6 +75,9 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
         for (int fc = 0; fc < 2; ++fc)
             if (!(p->wall_contact_angle[a][fc] >= 0.0 && p->wall_contact_angle[a][fc] <= 180.0))
                 return fail(TCP_EINVAL, "wall_contact_angle must lie in [0, 180] degrees (default 90, see tcp_params_default)");
+    if (p->hydro_lattice != 27 && p->hydro_lattice != 19) return fail(TCP_EINVAL, "hydro_lattice must be 27 or 19 (default 27, see tcp_params_default)");
+    if (p->hydro_lattice == 19 && p->s_high != 1.0 && !p->high_rate_equals_shear)
+        return fail(TCP_EUNSUPPORTED, "hydro_lattice = 19: the closed-form central-moment collision (s_high = 1) and BGK only; general rates need the D3Q27 basis");
     if (p->high_rate_equals_shear != 0 && p->high_rate_equals_shear != 1) return fail(TCP_EINVAL, "high_rate_equals_shear must be 0 or 1");
     return TCP_OK;
 }
@@ -89,7 +92,7 @@ Layout make_layout(int nx, int ny, int nz, const tcp_params* p) {
     auto take = [&](size_t count) { size_t o = off; off = align_up(off + count * es); return o; };
     const bool aa = p->streaming == TCP_STREAM_AA;      // in-place streaming: one grid of populations
     for (int b = 0; b < 2; ++b) L.h[b] = (aa && b) ? L.h[0] : take(27 * N);
-    for (int b = 0; b < 2; ++b) L.g[b] = (aa && b) ? L.g[0] : take(27 * N);
+    for (int b = 0; b < 2; ++b) L.g[b] = (aa && b) ? L.g[0] : take((size_t)p->hydro_lattice * N);
     for (int b = 0; b < 2; ++b) L.f[b] = QT ? ((aa && b) ? L.f[0] : take((size_t)QT * N)) : 0;
     for (int b = 0; b < 2; ++b) L.phi[b] = take(N);
     for (int b = 0; b < 2; ++b) L.T[b] = take(N);
@@ -355,15 +358,17 @@ int launch_fused(tcp_sim* s, const tcp::StepArgs<real>& A) {
     tcp::FusedCfg c;
     c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next; c.device = s->device;
     c.grid = grid_for((size_t)(A.cell1 - A.cell0));
+    const bool q19 = s->P.hydro_lattice == 19;       // D3Q19 hydrodynamic lattice: kernels of the *_q19 translation units
     if constexpr (sizeof(real) == 4) {
         if (s->use_pair && mode == 0) {
-            CK(s->walls ? tcp::launch_pair_walls(c, A, s->stream) : tcp::launch_pair_periodic(c, A, s->stream));
-        } else {
-            CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
+            if (q19) CK(s->walls ? tcp::launch_pair_walls_q19(c, A, s->stream) : tcp::launch_pair_periodic_q19(c, A, s->stream));
+            else CK(s->walls ? tcp::launch_pair_walls(c, A, s->stream) : tcp::launch_pair_periodic(c, A, s->stream));
+            s->launches++;
+            return TCP_OK;
         }
-    } else {
-        CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
     }
+    if (q19) CK(s->walls ? tcp::launch_fused_walls_q19(c, A, s->stream) : tcp::launch_fused_periodic_q19(c, A, s->stream));
+    else CK(s->walls ? tcp::launch_fused_walls(c, A, s->stream) : tcp::launch_fused_periodic(c, A, s->stream));
     s->launches++;
     return TCP_OK;
 }
@@ -411,8 +416,9 @@ int phase_message(const tcp_sim* s, int p, int dir, real* fields[32]) {
     }
     for (int q = 0; q < 27; ++q)
         if (tcp::cz27(q) == dir) fields[m++] = ptr<real>(s, s->L.h[o]) + q * N;
-    for (int q = 0; q < 27; ++q)
-        if (tcp::cz27(q) == dir) fields[m++] = ptr<real>(s, s->L.g[o]) + q * N;
+    const int QH = s->P.hydro_lattice;
+    for (int k = 0; k < QH; ++k)
+        if (tcp::cz27(tcp::q_of(QH, k)) == dir) fields[m++] = ptr<real>(s, s->L.g[o]) + k * N;
     const int QT = thermal_q(s->P.thermal);
     for (int k = 0; k < QT; ++k)
         if (tcp::cz27(tcp::q_of(QT, k)) == dir) fields[m++] = ptr<real>(s, s->L.f[oT]) + k * N;
@@ -554,12 +560,22 @@ int init_fields_t(tcp_sim* s, const void* phi, const void* u, const void* T) {
     tcp::StepArgs<real> A = make_args<real>(s);
     A.h_out = ptr<real>(s, s->L.h[0]); A.g_out = ptr<real>(s, s->L.g[0]); A.f_out = ptr<real>(s, s->L.f[0]);
     const unsigned grid = grid_for(N);
-    switch (thermal_q(s->P.thermal)) {
-    case 7: tcp::init_kernel<real, 7><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 15: tcp::init_kernel<real, 15><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 19: tcp::init_kernel<real, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    case 27: tcp::init_kernel<real, 27><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
-    default: tcp::init_kernel<real, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+    if (s->P.hydro_lattice == 19) {
+        switch (thermal_q(s->P.thermal)) {
+        case 7: tcp::init_kernel<real, 7, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        case 15: tcp::init_kernel<real, 15, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        case 19: tcp::init_kernel<real, 19, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        case 27: tcp::init_kernel<real, 27, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        default: tcp::init_kernel<real, 0, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        }
+    } else {
+        switch (thermal_q(s->P.thermal)) {
+        case 7: tcp::init_kernel<real, 7><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        case 15: tcp::init_kernel<real, 15><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        case 19: tcp::init_kernel<real, 19><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        case 27: tcp::init_kernel<real, 27><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        default: tcp::init_kernel<real, 0><<<grid, tcp::kBlock, 0, s->stream>>>(A); break;
+        }
     }
     s->launches++;
     CK(cudaGetLastError());
@@ -603,6 +619,23 @@ int fill_wall(tcp_sim* s, int axis, int face, const void* Tw) {
     return TCP_OK;
 }
 
+// p = c_s^2 rho(phi) sum_i g~_i into `out` (device memory, N values): natural layout, or the pushed layout of AA streaming
+template <typename real>
+void launch_pressure(tcp_sim* s, real* out) {
+    const size_t N = s->N;
+    const real* phi = ptr<real>(s, s->L.phi[s->cur]);
+    const real rho_L = (real)s->P.rho_L, drho = (real)(s->P.rho_H - s->P.rho_L);
+    const bool q19 = s->P.hydro_lattice == 19;
+    if (s->aa_next == 1) {   // AA, populations in the pushed layout (after init or an odd step)
+        if (q19) tcp::pressure_pushed_kernel<real, 19><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(make_args<real>(s), ptr<real>(s, s->L.g[0]), phi, out);
+        else tcp::pressure_pushed_kernel<real, 27><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(make_args<real>(s), ptr<real>(s, s->L.g[0]), phi, out);
+    } else {
+        if (q19) tcp::pressure_kernel<real, 19><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(ptr<real>(s, s->L.g[s->cur]), phi, out, (int)N, rho_L, drho);
+        else tcp::pressure_kernel<real, 27><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(ptr<real>(s, s->L.g[s->cur]), phi, out, (int)N, rho_L, drho);
+    }
+    s->launches++;
+}
+
 template <typename real>
 int read_fields_t(tcp_sim* s, void* phi, void* u, void* p, void* T) {
     const size_t N = s->N, es = sizeof(real);
@@ -611,14 +644,7 @@ int read_fields_t(tcp_sim* s, void* phi, void* u, void* p, void* T) {
     if (T) CK(cudaMemcpyAsync(T, ptr<real>(s, s->L.T[s->curT]), N * es, cudaMemcpyDefault, s->stream));
     if (p) {
         real* scratch = ptr<real>(s, s->L.phi[1 - s->cur]);   // free between steps
-        if (s->aa_next == 1)   // AA, populations in the pushed layout (after init or an odd step)
-            tcp::pressure_pushed_kernel<real><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(make_args<real>(s), ptr<real>(s, s->L.g[0]),
-                                                                                        ptr<real>(s, s->L.phi[s->cur]), scratch);
-        else
-            tcp::pressure_kernel<real><<<grid_for(N), tcp::kBlock, 0, s->stream>>>(ptr<real>(s, s->L.g[s->cur]), ptr<real>(s, s->L.phi[s->cur]),
-                                                                                   scratch, (int)N, (real)s->P.rho_L,
-                                                                                   (real)(s->P.rho_H - s->P.rho_L));
-        s->launches++;
+        launch_pressure<real>(s, scratch);
         CK(cudaGetLastError());
         CK(cudaMemcpyAsync(p, scratch, N * es, cudaMemcpyDefault, s->stream));
     }
@@ -707,6 +733,7 @@ int tcp_params_default(tcp_params* p) {
     p->s_bulk = p->s_high = 1.0;
     p->eps_normal = 1e-32;
     for (int a = 0; a < 3; ++a) p->wall_contact_angle[a][0] = p->wall_contact_angle[a][1] = 90.0;
+    p->hydro_lattice = 27;
     return TCP_OK;
 }
 
@@ -826,7 +853,7 @@ int tcp_halo_message_bytes(const tcp_sim* s, int phase, size_t* bytes) {
     if (!s || !bytes) return fail(TCP_EINVAL, "NULL argument");
     if (phase < 0 || phase >= halo_phases(s)) return fail(TCP_EINVAL, "phase out of range (tcp_halo_phases)");
     const int QT = thermal_q(s->P.thermal);
-    const size_t planes = phase > 0 ? 1 : 9 + 9 + (size_t)tcp::halo_crossing(QT, 1) + 1 + (QT ? 1 : 0) + (rk_first_stage_fused(s) ? 1 : 0);
+    const size_t planes = phase > 0 ? 1 : 9 + (size_t)tcp::halo_crossing(s->P.hydro_lattice, 1) + (size_t)tcp::halo_crossing(QT, 1) + 1 + (QT ? 1 : 0) + (rk_first_stage_fused(s) ? 1 : 0);
     *bytes = planes * s->nx * s->ny * (s->P.precision == TCP_F64 ? 8 : 4);
     return TCP_OK;
 }
@@ -887,22 +914,8 @@ int tcp_read_pressure_static(tcp_sim* s, void* p) {
         scratch = addr;
     }
     // every entry of [0, N) is written by the kernel before the copy reads it: the last call's contents never show
-    if (s->P.precision == TCP_F64) {
-        double* out = static_cast<double*>(scratch);
-        if (s->aa_next == 1)
-            tcp::pressure_pushed_kernel<double><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(make_args<double>(s), ptr<double>(s, s->L.g[0]), ptr<double>(s, s->L.phi[s->cur]), out);
-        else
-            tcp::pressure_kernel<double><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(ptr<double>(s, s->L.g[s->cur]), ptr<double>(s, s->L.phi[s->cur]), out, (int)s->N,
-                                                                                     s->P.rho_L, s->P.rho_H - s->P.rho_L);
-    } else {
-        float* out = static_cast<float*>(scratch);
-        if (s->aa_next == 1)
-            tcp::pressure_pushed_kernel<float><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(make_args<float>(s), ptr<float>(s, s->L.g[0]), ptr<float>(s, s->L.phi[s->cur]), out);
-        else
-            tcp::pressure_kernel<float><<<grid_for(s->N), tcp::kBlock, 0, s->stream>>>(ptr<float>(s, s->L.g[s->cur]), ptr<float>(s, s->L.phi[s->cur]), out, (int)s->N,
-                                                                                   (float)s->P.rho_L, (float)(s->P.rho_H - s->P.rho_L));
-    }
-    s->launches++;
+    if (s->P.precision == TCP_F64) launch_pressure<double>(s, static_cast<double*>(scratch));
+    else launch_pressure<float>(s, static_cast<float*>(scratch));
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(p, scratch, s->N * es, cudaMemcpyDefault, s->stream));
     CK(cudaStreamSynchronize(s->stream));

@@ -173,7 +173,7 @@ __device__ __forceinline__ real wall_temperature(const StepArgs<real>& A, const 
 // moving wall (reading S18): a population of direction (cx,cy,cz) that arrives at the cell
 // from a wall moving with U_w is the bounced one plus 2 w (c . U_w) / c_s^2 (hydrodynamic lattice only;
 // velocity-based model, no density factor).  (ox,oy,oz) = direction in which the wall lies (= -c).
-template <typename real, bool WALLS>
+template <typename real, bool WALLS, int QH = 27>
 __device__ __forceinline__ real wall_velocity_term(const StepArgs<real>& A, const Nbh<WALLS>& nb, int q27i) {
     if (!WALLS || !A.moving) return real(0);
     const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
@@ -181,7 +181,7 @@ __device__ __forceinline__ real wall_velocity_term(const StepArgs<real>& A, cons
     const int ax = nb.crossed(-cx, -cy, -cz, face);
     if (ax < 0) return real(0);
     const real* U = A.wall_u[ax][face];
-    return real(6.0 * weight(27, cls27(q27i))) * (real(cx) * U[0] + real(cy) * U[1] + real(cz) * U[2]);
+    return real(6.0 * weight(QH, cls27(q27i))) * (real(cx) * U[0] + real(cy) * U[1] + real(cz) * U[2]);
 }
 
 // Wetting boundary condition (refs. [34], [35]; reading S20): ghost value of phi behind a wall with
@@ -344,12 +344,14 @@ struct R1D {
 // force populations (ref. [20]), merged:
 //   scalar (h, f):  A0 = s - 1.5 u.b,  v = s u + a/2,  b = s u + a
 //   hydro  (g):     A0 = p* - 1.5 u.b, v = u + a/2,    b = u + a
-template <typename real>
+// Q = 27, or 19 (D3Q19 hydrodynamic lattice: its weights, the eight corner entries of out[] are set to 0).
+template <typename real, int Q = 27>
 __device__ __forceinline__ void equilibrium_plus_half_force27(real A0, const real u[3], const real v[3], const real b[3], real out[27]) {
 #pragma unroll
     for (int q = 0; q < 13; ++q) {
         const int cx = cx27(q), cy = cy27(q), cz = cz27(q);
-        const real w = real(weight(27, cls27(q)));
+        if (!has_class(Q, cls27(q))) { out[q] = real(0); out[26 - q] = real(0); continue; }
+        const real w = real(weight(Q, cls27(q)));
         const real cu = real(cx) * u[0] + real(cy) * u[1] + real(cz) * u[2];
         const real cb = real(cx) * b[0] + real(cy) * b[1] + real(cz) * b[2];
         const real cv = real(cx) * v[0] + real(cy) * v[1] + real(cz) * v[2];
@@ -358,7 +360,7 @@ __device__ __forceinline__ void equilibrium_plus_half_force27(real A0, const rea
         out[q] = sym + asym;
         out[26 - q] = sym - asym;
     }
-    out[13] = real(weight(27, 0)) * A0;
+    out[13] = real(weight(Q, 0)) * A0;
 }
 
 // out_q += sum_alpha m_alpha R^alpha_q(u): populations whose first-order central moments are m and
@@ -402,6 +404,48 @@ __device__ __forceinline__ void add_second_order27(real Axx, real Ayy, real Azz,
 #pragma unroll
             for (int x = 0; x < 3; ++x)
                 out[9 * z + 3 * y + x] += rz.r0[z] * P[y][x] + rz.r1[z] * Qm[y][x] + r2[z] * W[y][x];
+}
+
+// D3Q19 (hydrodynamic lattice, basis of reading S2: the monomials x^a y^b z^c, a, b, c <= 2, abc = 0):
+// out_q += populations whose second-order central moments are A_{alpha beta} and whose other basis central moments
+// vanish.  Their raw moments over the basis are M_b = 1/2 sum_{alpha beta} A_{alpha beta} d_alpha d_beta b (u) (Taylor
+// expansion of b(u + xi); the derivatives of a basis monomial are basis monomials, so no uncontrolled moment enters):
+//   x_a^2: A_aa;  x_a x_b: A_ab;  x_a^2 x_b: A_aa u_b + 2 A_ab u_a;  x_a^2 x_b^2: A_aa u_b^2 + A_bb u_a^2 + 4 A_ab u_a u_b,
+// and the populations follow from the lattice's raw-moment inversion (rest, 6 axis, 12 diagonal velocities), the same
+// one add_first_order_thermal<19> uses.  Entries of out[] at the eight corner velocities are left untouched.
+template <typename real>
+__device__ __forceinline__ void add_second_order19(real Axx, real Ayy, real Azz, real Axy, real Axz, real Ayz, const real u[3], real out[27]) {
+    const real Ad[3] = {Axx, Ayy, Azz}, Ao[3] = {Axy, Axz, Ayz};   // pair index p: 0 = (x,y), 1 = (x,z), 2 = (y,z)
+    real m22[3], m12[3], m21[3];
+#pragma unroll
+    for (int p = 0; p < 3; ++p) {
+        const int a = (p == 2 ? 1 : 0), b = (p == 0 ? 1 : 2);
+        m21[p] = Ad[a] * u[b] + real(2) * Ao[p] * u[a];                                  // x_a^2 x_b
+        m12[p] = Ad[b] * u[a] + real(2) * Ao[p] * u[b];                                  // x_a x_b^2
+        m22[p] = Ad[a] * u[b] * u[b] + Ad[b] * u[a] * u[a] + real(4) * Ao[p] * u[a] * u[b];
+    }
+    out[13] += -(Axx + Ayy + Azz) + (m22[0] + m22[1] + m22[2]);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        // the two pairs containing axis a and, in each, the moment of x_a x_other^2
+        const int p1 = (a == 2 ? 1 : 0), p2 = (a == 0 ? 1 : 2);
+        const real q1 = (a == 0) ? m12[0] : (a == 1 ? m21[0] : m21[1]);
+        const real q2 = (a == 0) ? m12[1] : (a == 1 ? m12[2] : m21[2]);
+        const real sym = real(0.5) * (Ad[a] - m22[p1] - m22[p2]), asym = real(-0.5) * (q1 + q2);
+        const int qp = 13 + (a == 0 ? 1 : (a == 1 ? 3 : 9));
+        out[qp] += sym + asym;
+        out[26 - qp] += sym - asym;
+    }
+#pragma unroll
+    for (int p = 0; p < 3; ++p) {
+        const int a = (p == 2 ? 1 : 0), b = (p == 0 ? 1 : 2);
+        const int sa = (a == 0 ? 1 : 3), sb = (b == 1 ? 3 : 9);                          // index strides of the two axes
+#pragma unroll
+        for (int ca = -1; ca <= 1; ca += 2)
+#pragma unroll
+            for (int cb = -1; cb <= 1; cb += 2)
+                out[13 + ca * sa + cb * sb] += real(0.25) * (m22[p] + real(ca) * m12[p] + real(cb) * m21[p] + real(ca * cb) * Ao[p]);
+    }
 }
 
 }  // namespace tcp

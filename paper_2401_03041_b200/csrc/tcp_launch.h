@@ -27,6 +27,14 @@ cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<float>& A, cuda
 cudaError_t launch_pair_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
 cudaError_t launch_pair_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
 
+// the same with the D3Q19 hydrodynamic lattice (tcp_params::hydro_lattice = 19; c.mode 0 or 1 only)
+cudaError_t launch_fused_periodic_q19(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
+cudaError_t launch_fused_periodic_q19(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+cudaError_t launch_fused_walls_q19(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
+cudaError_t launch_fused_walls_q19(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+cudaError_t launch_pair_periodic_q19(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+cudaError_t launch_pair_walls_q19(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);
+
 // thermal LB update alone (tcp_relax_temperature); c.mode 0 / 1, c.aa as above
 cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<double>& A, cudaStream_t stream);
 cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream);

@@ -1,4 +1,9 @@
-// Included by tcp_fused_f64.cu / tcp_fused_f32.cu with TCP_REAL defined.
+// Included by the tcp_fused_*.cu translation units with TCP_REAL defined (and TCP_WALLS_ONLY, TCP_PAIR, TCP_QH).
+// TCP_QH = 19 builds the kernels of the D3Q19 hydrodynamic lattice under the names launch_*_q19 (closed-form central-moment
+// and BGK collisions only; no calibration kernel, no thermal-only kernel: those do not depend on the hydrodynamic lattice).
+#ifndef TCP_QH
+#define TCP_QH 27
+#endif
 #include "tcp_launch.h"
 #include "tcp_step.cuh"
 #ifdef TCP_PAIR
@@ -10,8 +15,8 @@ namespace {
 
 template <typename real, int QT, bool WALLS, int MODE, int AA>
 cudaError_t launch_staged(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
-    const size_t smem = (size_t)(54 + QT - (h_direct<real, QT, AA>() ? 27 : 0)) * kBlock * sizeof(real);
-    auto kern = fused_step_async_kernel<real, QT, WALLS, MODE, AA>;
+    const size_t smem = (size_t)(27 + TCP_QH + QT - (h_direct<real, QT, AA>() ? 27 : 0)) * kBlock * sizeof(real);
+    auto kern = fused_step_async_kernel<real, QT, WALLS, MODE, AA, TCP_QH>;
     static bool configured[kMaxDevices] = {};   // once per instantiation and device: saves ~1 us per launch
     if (!configured[c.device]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -24,20 +29,25 @@ cudaError_t launch_staged(const FusedCfg& c, const StepArgs<real>& A, cudaStream
 
 template <typename real, int QT, bool WALLS>
 cudaError_t dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
+#if TCP_QH == 27
     if (c.mode == 3) {   // roofline calibration kernel (tcp_pattern_copy_ms): two-grid, periodic only
         if constexpr (!WALLS) return launch_staged<real, QT, false, 3, 0>(c, A, stream);
         else return cudaErrorNotSupported;
     }
+#endif
     switch (3 * c.aa + c.mode) {   // c.aa: 0 two-grid, 1 AA even step, 2 AA odd step
     case 0: return launch_staged<real, QT, WALLS, 0, 0>(c, A, stream);
     case 1: return launch_staged<real, QT, WALLS, 1, 0>(c, A, stream);
-    case 2: return launch_staged<real, QT, WALLS, 2, 0>(c, A, stream);
     case 3: return launch_staged<real, QT, WALLS, 0, 1>(c, A, stream);
     case 4: return launch_staged<real, QT, WALLS, 1, 1>(c, A, stream);
-    case 5: return launch_staged<real, QT, WALLS, 2, 1>(c, A, stream);
     case 6: return launch_staged<real, QT, WALLS, 0, 2>(c, A, stream);
     case 7: return launch_staged<real, QT, WALLS, 1, 2>(c, A, stream);
-    default: return launch_staged<real, QT, WALLS, 2, 2>(c, A, stream);
+#if TCP_QH == 27   // general central-moment rates: tensor-product D3Q27 basis only
+    case 2: return launch_staged<real, QT, WALLS, 2, 0>(c, A, stream);
+    case 5: return launch_staged<real, QT, WALLS, 2, 1>(c, A, stream);
+    case 8: return launch_staged<real, QT, WALLS, 2, 2>(c, A, stream);
+#endif
+    default: return cudaErrorNotSupported;
     }
 }
 
@@ -52,6 +62,7 @@ cudaError_t by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t 
     }
 }
 
+#if TCP_QH == 27
 template <typename real, int QT, bool WALLS>
 cudaError_t thermal_dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
     switch (2 * c.aa + (c.mode == 1)) {
@@ -74,13 +85,14 @@ cudaError_t thermal_by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaS
     default: return cudaErrorInvalidValue;
     }
 }
+#endif
 
 #ifdef TCP_PAIR
 // packed-pair single-precision kernels (tcp_pair.cuh)
 template <int QT, bool WALLS, int MODE, int AA>
 cudaError_t launch_pair(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_t stream) {
-    const size_t smem = (size_t)(54 + QT - (pair_h_direct<QT, AA>() ? 27 : 0)) * kBlock * sizeof(float2);
-    auto kern = fused_step_pair_kernel<QT, WALLS, MODE, AA>;
+    const size_t smem = (size_t)(27 + TCP_QH + QT - (pair_h_direct<QT, AA>() ? 27 : 0)) * kBlock * sizeof(float2);
+    auto kern = fused_step_pair_kernel<QT, WALLS, MODE, AA, TCP_QH>;
     static bool configured[kMaxDevices] = {};
     if (!configured[c.device]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -114,20 +126,30 @@ cudaError_t pair_by_stencil(const FusedCfg& c, const StepArgs<float>& Af, cudaSt
 
 }  // namespace
 
+#if TCP_QH == 27
+#define TCP_NAME(n) n
+#else
+#define TCP_NAME(n) n##_q19
+#endif
+
 #ifdef TCP_PAIR
 #ifdef TCP_WALLS_ONLY
-cudaError_t launch_pair_walls(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream) { return pair_by_stencil<true>(c, A, stream); }
+cudaError_t TCP_NAME(launch_pair_walls)(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream) { return pair_by_stencil<true>(c, A, stream); }
 #else
-cudaError_t launch_pair_periodic(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream) { return pair_by_stencil<false>(c, A, stream); }
+cudaError_t TCP_NAME(launch_pair_periodic)(const FusedCfg& c, const StepArgs<float>& A, cudaStream_t stream) { return pair_by_stencil<false>(c, A, stream); }
 #endif
 #endif
 
 #ifdef TCP_WALLS_ONLY
-cudaError_t launch_fused_walls(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, true>(c, A, stream); }
+cudaError_t TCP_NAME(launch_fused_walls)(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, true>(c, A, stream); }
+#if TCP_QH == 27
 cudaError_t launch_thermal_walls(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return thermal_by_stencil<TCP_REAL, true>(c, A, stream); }
+#endif
 #else
-cudaError_t launch_fused_periodic(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, false>(c, A, stream); }
+cudaError_t TCP_NAME(launch_fused_periodic)(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return by_stencil<TCP_REAL, false>(c, A, stream); }
+#if TCP_QH == 27
 cudaError_t launch_thermal_periodic(const FusedCfg& c, const StepArgs<TCP_REAL>& A, cudaStream_t stream) { return thermal_by_stencil<TCP_REAL, false>(c, A, stream); }
+#endif
 #endif
 
 }  // namespace tcp

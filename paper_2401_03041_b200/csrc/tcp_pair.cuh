@@ -67,7 +67,7 @@ __device__ __forceinline__ f32x2 wall_temperature_pair(const StepArgs<f32x2>& A,
     const float* plane = A.wallT[axis][face];
     return f32x2(plane[base + xa], plane[base + xb]);
 }
-template <bool WALLS>
+template <bool WALLS, int QH = 27>
 __device__ __forceinline__ f32x2 wall_velocity_term_pair(const StepArgs<f32x2>& A, const NbhPair<WALLS>& nb, int q27i) {
     if (!WALLS || !A.moving) return f32x2(0.0f);
     const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
@@ -75,7 +75,7 @@ __device__ __forceinline__ f32x2 wall_velocity_term_pair(const StepArgs<f32x2>& 
     const int ax = nb.crossed(-cy, -cz, face);
     if (ax < 0) return f32x2(0.0f);
     const float* U = A.wall_u[ax][face];
-    return f32x2((float)(6.0 * weight(27, cls27(q27i))) * ((float)cx * U[0] + (float)cy * U[1] + (float)cz * U[2]));
+    return f32x2((float)(6.0 * weight(QH, cls27(q27i))) * ((float)cx * U[0] + (float)cy * U[1] + (float)cz * U[2]));
 }
 
 __device__ __forceinline__ void cp_async_4(float* sdst, const float* gsrc) {
@@ -147,7 +147,7 @@ __host__ __device__ constexpr bool pair_h_direct() { return TCP_PAIR_HDIRECT && 
 template <int QT, int AA = 0>
 __host__ __device__ constexpr int pair_min_blocks() { return (QT >= 15 && !pair_h_direct<QT, AA>()) ? 2 : TCP_MINB; }
 
-template <int QT, bool WALLS, int MODE, int AA>
+template <int QT, bool WALLS, int MODE, int AA, int QH = 27>
 __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_pair_kernel(const StepArgs<f32x2> A) {
     using real = f32x2;
     extern __shared__ __align__(16) unsigned char smem_raw_pair[];
@@ -213,11 +213,10 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
         for (int q = 0; q < 27; ++q) issue(stage + q * kBlock, A.h_in, 27, q, q);
     }
     cp_async_commit();
-#pragma unroll
-    for (int q = 0; q < 27; ++q) issue(stage + (SO + 27 + q) * kBlock, A.g_in, 27, q, q);
+    static_for<0, QH>([&](auto K) { constexpr int k = decltype(K)::value; issue(stage + (SO + 27 + k) * kBlock, A.g_in, QH, k, q_of(QH, k)); });
     cp_async_commit();
     if constexpr (QT > 0)
-        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; issue(stage + (SO + 54 + k) * kBlock, A.f_in, QT, k, q_of(QT, k)); });
+        static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; issue(stage + (SO + 27 + QH + k) * kBlock, A.f_in, QT, k, q_of(QT, k)); });
     cp_async_commit();
 
     real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
@@ -227,7 +226,7 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
 #pragma unroll
     for (int al = 0; al < 3; ++al) { const float2 t = *reinterpret_cast<const float2*>(A.u + al * N + cell); u[al] = real(t.x, t.y); }
 
-    prefetch_next_wave<float, QT, AA, StepArgs<f32x2>>(A, 2 * kBlock, pair_min_blocks<QT, AA>());
+    prefetch_next_wave<float, QT, AA, QH, StepArgs<f32x2>>(A, 2 * kBlock, pair_min_blocks<QT, AA>());
 
     real phi_new;
     {
@@ -245,22 +244,25 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
     {
         cp_async_wait<1>();
         real g[27];
+        if constexpr (QH != 27) {
 #pragma unroll
-        for (int q = 0; q < 27; ++q) g[q].v = stage[(SO + 27 + q) * kBlock];
-        if (WALLS && aa != 1 && A.moving) {
-#pragma unroll
-            for (int q = 0; q < 27; ++q) g[q] += wall_velocity_term_pair(A, nb, q);
+            for (int q = 0; q < 27; ++q) g[q] = real(0.0f);   // velocities the hydrodynamic lattice does not have
         }
-        collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+        static_for<0, QH>([&](auto K) {
+            constexpr int k = decltype(K)::value, q = q_of(QH, k);
+            g[q].v = stage[(SO + 27 + k) * kBlock];
+            if (WALLS && aa != 1 && A.moving) g[q] += wall_velocity_term_pair<WALLS, QH>(A, nb, q);
+        });
+        collide_hydro<real, MODE, QH>(A, g, phi_c, G, lapPhi, T_c, Th, u);
         if (active) {
-#pragma unroll
-            for (int q = 0; q < 27; ++q) {
+            static_for<0, QH>([&](auto K) {
+                constexpr int k = decltype(K)::value, q = q_of(QH, k);
                 // AA odd step, link into a moving wall: what comes back is direction opp(q) with its wall term
                 int face = 0;
                 const bool into_wall = WALLS && aa == 2 && nb.crossed(cy27(q), cz27(q), face) >= 0;
                 bool wl;
-                put(A.g_out, 27, q, q, into_wall ? g[q] + wall_velocity_term_pair(A, nb, 26 - q) : g[q], wl);
-            }
+                put(A.g_out, QH, k, q, into_wall ? g[q] + wall_velocity_term_pair<WALLS, QH>(A, nb, 26 - q) : g[q], wl);
+            });
 #pragma unroll
             for (int al = 0; al < 3; ++al) *reinterpret_cast<float2*>(A.u + al * N + cell) = u[al].v;
         }
@@ -281,7 +283,7 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
             int face = 0;
             const int ax = aa == 1 ? -1 : nb.crossed(-cy27(q), -cz27(q), face);
-            real v; v.v = stage[(SO + 54 + k) * kBlock];
+            real v; v.v = stage[(SO + 27 + QH + k) * kBlock];
             if (WALLS && ax >= 0)   // anti-bounce-back (S9): T_w at the tangential position of each lane's source cell
                 v = real(2.0 * weight(QT, cls27(q))) * wall_temperature_pair(A, nb, ax, face, -cx27(q), -cy27(q), -cz27(q)) - v;
             f[k] = v;

@@ -139,7 +139,8 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
 
 // ---- hydrodynamic LB on one cell: eqs. 16-22, forces of eqs. 7-9 -------------------------------
 // g = pulled populations; phi_c, G, lapPhi from phi^n (S16); T_c, Th = grad T^n.  Writes g~, u^{n+1}.
-template <typename real, int MODE>
+// QH = 27 or 19 (D3Q19 hydrodynamic lattice): g[] stays indexed as D3Q27 with the eight corner entries 0.
+template <typename real, int MODE, int QH = 27>
 __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27], real phi_c, const real G[3], real lapPhi,
                                               real T_c, const real Th[3], real u[3]) {
     const Mom2<real> M = moments27<real, true>(g);
@@ -195,11 +196,12 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
     for (int al = 0; al < 3; ++al) { b[al] = u[al] + a[al]; v[al] = u[al] + real(0.5) * a[al]; }
     const real A0 = ps - real(1.5) * (u[0] * b[0] + u[1] * b[1] + u[2] * b[2]);
     real out[27];
-    equilibrium_plus_half_force27<real>(A0, u, v, b, out);
+    equilibrium_plus_half_force27<real, QH>(A0, u, v, b, out);
     if (MODE == 1) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = (real(1) - om) * g[q] + om * out[q];
     } else if (MODE == 2) {
+        static_assert(MODE != 2 || QH == 27, "general central-moment rates: the sweep transform exists for the tensor-product D3Q27 basis only");
         // general rates (s_high != 1): g~ = E + K^-1 (I - S) K X,  X = (g - g_eq) + F/2 = g - E(-a)
         // (I - S vanishes on orders 0 and 1).  K is applied as three sweeps of the 1-D central-moment
         // transform (x, y, z), its inverse as the reverse sweeps.
@@ -208,7 +210,7 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
             real bm[3], vm[3];
 #pragma unroll
             for (int al = 0; al < 3; ++al) { bm[al] = u[al] - a[al]; vm[al] = u[al] - real(0.5) * a[al]; }
-            equilibrium_plus_half_force27<real>(ps - real(1.5) * (u[0] * bm[0] + u[1] * bm[1] + u[2] * bm[2]), u, vm, bm, X);
+            equilibrium_plus_half_force27<real, QH>(ps - real(1.5) * (u[0] * bm[0] + u[1] * bm[1] + u[2] * bm[2]), u, vm, bm, X);
 #pragma unroll
             for (int q = 0; q < 27; ++q) X[q] = g[q] - X[q];
         }
@@ -238,9 +240,13 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
         const real tr3 = (kxx + kyy + kzz) * real(1.0 / 3.0);
         const real k2 = real(1) - om, kb = (real(1) - A.s_bulk) * tr3;
         kxx = k2 * (kxx - tr3) + kb; kyy = k2 * (kyy - tr3) + kb; kzz = k2 * (kzz - tr3) + kb;
-        R1D<real> rx, ry, rz;
-        rx.set(u[0]); ry.set(u[1]); rz.set(u[2]);
-        add_second_order27<real>(kxx, kyy, kzz, k2 * kxy, k2 * kxz, k2 * kyz, rx, ry, rz, out);
+        if constexpr (QH == 27) {
+            R1D<real> rx, ry, rz;
+            rx.set(u[0]); ry.set(u[1]); rz.set(u[2]);
+            add_second_order27<real>(kxx, kyy, kzz, k2 * kxy, k2 * kxz, k2 * kyz, rx, ry, rz, out);
+        } else {
+            add_second_order19<real>(kxx, kyy, kzz, k2 * kxy, k2 * kxz, k2 * kyz, u, out);
+        }
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = out[q];
     }
@@ -347,11 +353,11 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 #ifndef TCP_PF2
 #define TCP_PF2 40
 #endif
-template <typename elem, int QT, int AA, typename Args>
+template <typename elem, int QT, int AA, int QH = 27, typename Args>
 __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_block, int resident) {
     if constexpr (TCP_PF > 0) {
         if (threadIdx.x != 0) return;
-        constexpr int NP = 54 + QT, NR = NP + 7;
+        constexpr int NP = 27 + QH + QT, NR = NP + 7;
         unsigned nsm;
         asm("mov.u32 %0, %%nsmid;" : "=r"(nsm));
         const unsigned r = blockIdx.x % NR;
@@ -363,9 +369,11 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
         int q27i = 13, plane = 0, Q = 27;
         long long off = c0;
         if (r < 27) { base = A.h_in; plane = q27i = r; }
-        else if (r < 54) { base = A.g_in; plane = q27i = r - 27; }
-        else if (r < NP) {
-            base = A.f_in; plane = r - 54; Q = QT;
+        else if (r < 27 + QH) {
+            base = A.g_in; plane = r - 27; Q = QH;
+            static_for<0, QH>([&](auto K) { constexpr int k = decltype(K)::value; if (plane == k) q27i = q_of(QH, k); });
+        } else if (r < NP) {
+            base = A.f_in; plane = r - 27 - QH; Q = QT;
             static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; if (plane == k) q27i = q_of(QT, k); });
         } else {
             const int j = r - NP;
@@ -409,10 +417,10 @@ __host__ __device__ constexpr int async_min_blocks() {
     return (sizeof(real) == 8 && QT >= 15) ? 2 : TCP_MINB;
 }
 
-template <typename real, int QT, bool WALLS, int MODE, int AA>
+template <typename real, int QT, bool WALLS, int MODE, int AA, int QH = 27>
 __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT, AA>()) fused_step_async_kernel(const StepArgs<real> A) {
     extern __shared__ __align__(16) unsigned char smem_raw_async[];
-    real* stage = reinterpret_cast<real*>(smem_raw_async);     // [54 + QT][kBlock]
+    real* stage = reinterpret_cast<real*>(smem_raw_async);     // [27 + QH + QT][kBlock] (27 less if h is not staged)
     const int tid = threadIdx.x;
     const int gtid = A.cell0 + blockIdx.x * kBlock + tid;
     const bool active = gtid < A.cell1;
@@ -460,13 +468,15 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT, AA>()) fuse
         for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + q * kBlock + tid, src_of(A.h_in, 27, q, q));
     }
     cp_async_commit();
-#pragma unroll
-    for (int q = 0; q < 27; ++q) cp_async_elem<real>(stage + (SO + 27 + q) * kBlock + tid, src_of(A.g_in, 27, q, q));
+    static_for<0, QH>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(QH, k);
+        cp_async_elem<real>(stage + (SO + 27 + k) * kBlock + tid, src_of(A.g_in, QH, k, q));
+    });
     cp_async_commit();
     if constexpr (QT > 0) {
         static_for<0, QT>([&](auto K) {
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
-            cp_async_elem<real>(stage + (SO + 54 + k) * kBlock + tid, src_of(A.f_in, QT, k, q));
+            cp_async_elem<real>(stage + (SO + 27 + QH + k) * kBlock + tid, src_of(A.f_in, QT, k, q));
         });
     }
     cp_async_commit();
@@ -483,7 +493,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT, AA>()) fuse
     real u[3] = {A.u[cell], A.u[N + cell], A.u[2 * N + cell]};
 
     // (not in the calibration kernel: without arithmetic its blocks are too short-lived, measured 10.98 ms with against 10.5 ms without)
-    if constexpr (MODE != 3) prefetch_next_wave<real, QT, AA, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT, AA>());
+    if constexpr (MODE != 3) prefetch_next_wave<real, QT, AA, QH, StepArgs<real>>(A, kBlock, async_min_blocks<real, QT, AA>());
 
     real phi_new;
     {
@@ -501,21 +511,24 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT, AA>()) fuse
     {
         cp_async_wait<1>();
         real g[27];
+        if constexpr (QH != 27) {
 #pragma unroll
-        for (int q = 0; q < 27; ++q) g[q] = stage[(SO + 27 + q) * kBlock + tid];
-        if (WALLS && aa != 1 && A.moving) {
-#pragma unroll
-            for (int q = 0; q < 27; ++q) g[q] += wall_velocity_term<real, WALLS>(A, nb, q);
+            for (int q = 0; q < 27; ++q) g[q] = real(0);     // velocities the hydrodynamic lattice does not have
         }
-        if constexpr (MODE != 3) collide_hydro<real, MODE>(A, g, phi_c, G, lapPhi, T_c, Th, u);
+        static_for<0, QH>([&](auto K) {
+            constexpr int k = decltype(K)::value, q = q_of(QH, k);
+            g[q] = stage[(SO + 27 + k) * kBlock + tid];
+            if (WALLS && aa != 1 && A.moving) g[q] += wall_velocity_term<real, WALLS, QH>(A, nb, q);
+        });
+        if constexpr (MODE != 3) collide_hydro<real, MODE, QH>(A, g, phi_c, G, lapPhi, T_c, Th, u);
         if (active) {
-#pragma unroll
-            for (int q = 0; q < 27; ++q) {
+            static_for<0, QH>([&](auto K) {
+                constexpr int k = decltype(K)::value, q = q_of(QH, k);
                 bool wl;
-                real* dst = dst_of(A.g_out, 27, q, q, wl);
+                real* dst = dst_of(A.g_out, QH, k, q, wl);
                 // AA odd step, link into a moving wall: store what comes back, direction opp(q) with its wall term
-                *dst = (WALLS && wl) ? g[q] + wall_velocity_term<real, WALLS>(A, nb, 26 - q) : g[q];
-            }
+                *dst = (WALLS && wl) ? g[q] + wall_velocity_term<real, WALLS, QH>(A, nb, 26 - q) : g[q];
+            });
             A.u[cell] = u[0]; A.u[N + cell] = u[1]; A.u[2 * N + cell] = u[2];
         }
     }
@@ -533,7 +546,7 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT, AA>()) fuse
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
             int face = 0;
             const int ax = aa == 1 ? -1 : nb.crossed(-cx27(q), -cy27(q), -cz27(q), face);
-            const real v = stage[(SO + 54 + k) * kBlock + tid];
+            const real v = stage[(SO + 27 + QH + k) * kBlock + tid];
             if (WALLS && ax >= 0)   // anti-bounce-back (S9): the staged value is f~_opp of the own cell
                 f[k] = real(2.0 * weight(QT, cls27(q))) * wall_temperature(A, nb, ax, face, -cx27(q), -cy27(q), -cz27(q)) - v;
             else
@@ -665,7 +678,7 @@ struct RkArgs {
 };
 
 // ---- initialisation and read-back --------------------------------------------------------------
-template <typename real, int QT>
+template <typename real, int QT, int QH = 27>
 __global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
     const int cell = blockIdx.x * kBlock + threadIdx.x;
     if (cell >= A.ncell) return;
@@ -695,13 +708,13 @@ __global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.h_out, 27, q, q, wl) = out[q]; }
     }
-    equilibrium_plus_half_force27<real>(-real(1.5) * uu, u, u, u, out);                   // eq. 18, p* = 0
-#pragma unroll
-    for (int q = 0; q < 27; ++q) {
+    equilibrium_plus_half_force27<real, QH>(-real(1.5) * uu, u, u, u, out);               // eq. 18, p* = 0
+    static_for<0, QH>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(QH, k);
         bool wl;
-        real* dst = dst_of(A.g_out, 27, q, q, wl);
-        *dst = wl ? out[q] + wall_velocity_term<real, true>(A, nb, 26 - q) : out[q];
-    }
+        real* dst = dst_of(A.g_out, QH, k, q, wl);
+        *dst = wl ? out[q] + wall_velocity_term<real, true, QH>(A, nb, 26 - q) : out[q];
+    });
     if constexpr (QT > 0) {
         real f[QT];
         thermal_equilibrium<real, QT>(A.T_in[cell], u, f);
@@ -722,7 +735,7 @@ __global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
 
 // p = c_s^2 rho(phi) sum_q g~_q(x).  pushed = 1: AA layout after init / an odd step, where g~_q(x) sits in
 // plane q at x + c_q (plane opp(q) at x for a link into a wall).
-template <typename real>
+template <typename real, int QH = 27>
 __global__ void __launch_bounds__(kBlock) pressure_pushed_kernel(const StepArgs<real> A, const real* __restrict__ g, const real* __restrict__ phi,
                                                                 real* __restrict__ p) {
     const int cell = blockIdx.x * kBlock + threadIdx.x;
@@ -732,16 +745,16 @@ __global__ void __launch_bounds__(kBlock) pressure_pushed_kernel(const StepArgs<
     const int x = cell % A.nx, t = cell / A.nx;
     nb.init_xyz(A, x, t % A.ny, t / A.ny);
     real s = real(0);
-#pragma unroll
-    for (int q = 0; q < 27; ++q) {
+    static_for<0, QH>([&](auto K) {
+        constexpr int k = decltype(K)::value, q = q_of(QH, k);
         int face = 0;
         const bool wl = nb.crossed(cx27(q), cy27(q), cz27(q), face) >= 0;
-        s += wl ? g[(26 - q) * N + cell] : g[q * N + nb.at(cx27(q), cy27(q), cz27(q))];
-    }
+        s += wl ? g[(QH - 1 - k) * N + cell] : g[k * N + nb.at(cx27(q), cy27(q), cz27(q))];
+    });
     p[cell] = real(1.0 / 3.0) * (A.rho_L + phi[cell] * A.drho) * s;
 }
 
-template <typename real>
+template <typename real, int QH = 27>
 __global__ void __launch_bounds__(kBlock) pressure_kernel(const real* __restrict__ g, const real* __restrict__ phi, real* __restrict__ p,
                                                          int ncell, real rho_L, real drho) {
     const int cell = blockIdx.x * kBlock + threadIdx.x;
@@ -749,7 +762,7 @@ __global__ void __launch_bounds__(kBlock) pressure_kernel(const real* __restrict
     const long long N = ncell;
     real s = real(0);
 #pragma unroll
-    for (int q = 0; q < 27; ++q) s += g[q * N + cell];
+    for (int q = 0; q < QH; ++q) s += g[q * N + cell];
     p[cell] = real(1.0 / 3.0) * (rho_L + phi[cell] * drho) * s;
 }
 

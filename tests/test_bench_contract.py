@@ -25,6 +25,7 @@ def test_algorithmic_bytes_per_cell():
     assert bench.step_values_per_cell("rk2") * 8 == 936 + 8 + 56
     assert bench.step_values_per_cell("rk4") * 8 == 936 + 16 + 72 + 72 + 56
     assert bench.step_values_per_cell("lb_d3q7") * 8 == 1056
+    assert bench.step_values_per_cell("lb_d3q7", 19) * 8 == 928         # D3Q19 hydrodynamic lattice: 16 values less
 
 
 def test_benchmark_fluid_has_equal_conductivities():
@@ -59,7 +60,7 @@ def test_variants_cover_baseline_configs4_and_traffic_has_provenance():
     """The default line carries short device-timed runs of the other rows of BASELINE configs[4] (>= 7 entries: D3Q15/19/27,
     RK2, RK4, AA at 400^3 fp64, fp32 at 512^3, D3Q7 at 256^3); every ncu traffic figure names its commit and command."""
     assert len(bench.VARIANTS) >= 7
-    got = {(n, t, p) for (n, t, p, s) in bench.VARIANTS}
+    got = {(v[0], v[1], v[2]) for v in bench.VARIANTS}
     for need in ((400, "lb_d3q15", "f64"), (400, "lb_d3q19", "f64"), (400, "lb_d3q27", "f64"), (400, "rk2", "f64"),
                  (400, "rk4", "f64"), (512, "lb_d3q7", "f32"), (256, "lb_d3q7", "f64")):
         assert need in got

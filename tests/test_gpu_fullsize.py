@@ -48,11 +48,13 @@ def _sample_cells(wl, n, samples, rng):
     return picks
 
 
-def _sampled_parity(n, thermal, steps, samples, half, precision="f64", streaming="two_grid"):
+def _sampled_parity(n, thermal, steps, samples, half, precision="f64", streaming="two_grid", extra=None):
     """-> dict field -> (worst abs error over the samples, max |oracle| over the samples)"""
     assert half >= 2 * steps + 2
     wl = W.perf_box(n, thermal=thermal, device="cuda")
     tdt = torch.float64 if precision == "f64" else torch.float32
+    if extra:
+        wl.params.update(extra)
     sim = tcp.Simulation(n, n, n, dict(wl.params, precision=precision, streaming=streaming))
     sim.init_fields(wl.phi.to(tdt), None, wl.T.to(tdt))
     sim.step(steps)

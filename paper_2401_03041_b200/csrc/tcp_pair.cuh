@@ -204,6 +204,19 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
     };
     constexpr bool HD = pair_h_direct<QT, AA>();
     constexpr int SO = HD ? -27 : 0;
+    // The phi / T stencil loads and u.  With the D3Q7 thermal LB (two-grid) they are issued BEFORE the staged copies of g and f:
+    // the LSU works through its queue in order, the stencils and h are what the thread needs first, and 34 cp.async of 8 LSU
+    // cycles each would otherwise sit in front of them.  Measured sustained at 512^3: D3Q7 12.58-12.60 vs 13.00-13.05 ms; the
+    // other variants lose 1-2 % that way (RK2 12.51-12.53 vs 12.39-12.44, AA 13.68-13.71 vs 13.42-13.44, D3Q19 unchanged)
+    // and keep the stencils last; so does the fp64 kernel (D3Q7 11.98-12.00 vs 12.02-12.06, RK2 11.71-11.74 vs 11.34-11.38).
+    constexpr bool SF = QT == 7 && AA == 0;
+    real phi_c, G[3], lapPhi, T_c, Th[3], lapT, u[3];
+    auto load_fields = [&]() {
+        stencil27_pair<WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
+        stencil27_pair<WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
+#pragma unroll
+        for (int al = 0; al < 3; ++al) { const float2 t = *reinterpret_cast<const float2*>(A.u + al * N + cell); u[al] = real(t.x, t.y); }
+    };
     float2 hd[HD ? 27 : 1];
     if constexpr (HD) {
 #pragma unroll
@@ -213,18 +226,14 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
         for (int q = 0; q < 27; ++q) issue(stage + q * kBlock, A.h_in, 27, q, q);
     }
     cp_async_commit();
+    if constexpr (SF) load_fields();
     static_for<0, QH>([&](auto K) { constexpr int k = decltype(K)::value; issue(stage + (SO + 27 + k) * kBlock, A.g_in, QH, k, q_of(QH, k)); });
     cp_async_commit();
     if constexpr (QT > 0)
         static_for<0, QT>([&](auto K) { constexpr int k = decltype(K)::value; issue(stage + (SO + 27 + QH + k) * kBlock, A.f_in, QT, k, q_of(QT, k)); });
     cp_async_commit();
 
-    real phi_c, G[3], lapPhi, T_c, Th[3], lapT;
-    stencil27_pair<WALLS, false>(A, nb, A.phi_in, phi_c, G, lapPhi);
-    stencil27_pair<WALLS, true>(A, nb, A.T_in, T_c, Th, lapT);
-    real u[3];
-#pragma unroll
-    for (int al = 0; al < 3; ++al) { const float2 t = *reinterpret_cast<const float2*>(A.u + al * N + cell); u[al] = real(t.x, t.y); }
+    if constexpr (!SF) load_fields();
 
     prefetch_next_wave<float, QT, AA, QH, StepArgs<f32x2>>(A, 2 * kBlock, pair_min_blocks<QT, AA>());
 

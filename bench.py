@@ -263,7 +263,7 @@ def run_ours(args):
     value = aggregate_mlups(N, args.steps, world, ms_max)
     # roofline calibration: the same access pattern and staging with stencils and collisions removed
     pattern_ms = None
-    if rank == 0 and args.streaming == "two_grid" and QT[thermal]:   # calibrated for the one-kernel (thermal LB) step only
+    if rank == 0 and args.streaming == "two_grid" and QT[thermal] and args.hydro == 27:   # calibrated for the one-kernel (thermal LB) D3Q27 step only
         sim.pattern_copy_ms(3)
         pattern_ms = sim.pattern_copy_ms(max(5, min(args.steps, 20)))
     # ---- sustained figure: the same kernel for >= 3 s after the K-step region, with its own clock record.  The K-step

@@ -204,7 +204,7 @@ int tcp_last_step_ms(tcp_sim *s, float *ms);
  * spare phi / T buffers, so the simulation is unchanged -- except u, which is rewritten with itself.
  * It times itself with events of its own and is not counted by tcp_launch_count, so tcp_last_step_ms and
  * tcp_launch_count keep describing the method's kernels only.
- * Errors: TCP_ESTATE, TCP_EINVAL, TCP_EUNSUPPORTED (walls or AA streaming). */
+ * Errors: TCP_ESTATE, TCP_EINVAL, TCP_EUNSUPPORTED (walls, AA streaming, ghost planes, hydro_lattice = 19). */
 int tcp_pattern_copy_ms(tcp_sim *s, int nlaunches, float *ms);
 
 int tcp_destroy(tcp_sim *s);

@@ -926,8 +926,8 @@ int tcp_pattern_copy_ms(tcp_sim* s, int nlaunches, float* ms) {
     if (!s || !ms) return fail(TCP_EINVAL, "NULL argument");
     if (!s->initialised) return fail(TCP_ESTATE, "tcp_init_fields has not been called");
     if (nlaunches < 1) return fail(TCP_EINVAL, "nlaunches must be >= 1");
-    if (s->walls || s->P.streaming != TCP_STREAM_TWO_GRID || s->halo[0] || s->halo[1])
-        return fail(TCP_EUNSUPPORTED, "pattern copy: periodic two-grid simulations without ghost planes only");
+    if (s->walls || s->P.streaming != TCP_STREAM_TWO_GRID || s->halo[0] || s->halo[1] || s->P.hydro_lattice != 27)
+        return fail(TCP_EUNSUPPORTED, "pattern copy: periodic two-grid simulations without ghost planes and with the D3Q27 hydrodynamic lattice only");
     DeviceScope scope(s);
     tcp::FusedCfg c;
     c.qt = thermal_q(s->P.thermal); c.walls = false; c.mode = 3; c.aa = 0; c.device = s->device; c.grid = grid_for(s->N);

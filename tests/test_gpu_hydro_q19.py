@@ -81,6 +81,12 @@ def test_general_rates_are_refused_and_the_workspace_is_smaller():
     with pytest.raises(tcp.TcpError) as e:
         tcp.tcp_workspace_bytes(8, 8, 8, tcp.make_params(dict(hydro_lattice=15)))
     assert e.value.code == tcp.TCP_EINVAL
+    sim = tcp.Simulation(8, 8, 8, Q19)          # the calibration kernel exists for the D3Q27 layout only
+    sim.init_fields(np.zeros((8, 8, 8)))
+    with pytest.raises(tcp.TcpError) as e:
+        sim.pattern_copy_ms(1)
+    assert e.value.code == tcp.TCP_EUNSUPPORTED
+    sim.close()
     n = 64
     b27 = tcp.tcp_workspace_bytes(n, n, n, tcp.make_params({}))
     b19 = tcp.tcp_workspace_bytes(n, n, n, tcp.make_params(Q19))

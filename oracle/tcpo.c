@@ -69,6 +69,9 @@ typedef struct tcpo_params {
                                           (wetting boundary condition; reading S20); 90 = neutral = mirror ghost */
     int hydro_lattice;                 /* 27 (default) or 19: lattice of the hydrodynamic populations g ("hydrodynamic LBM solvers
                                           often rely on a D3Q19 or D3Q27 stencil"); weights App. B.3, basis S2 */
+    int collision_space;               /* 0 (default): central moments, K(u)_{m,i} = b_m(c_i - u); 1: raw moments, K(0) -- the
+                                          multiple-relaxation-time (MRT) operator with the same basis and rates ("the SRT or MRT methods
+                                          retain widespread usage") */
     /* ---- oracle-only switches (no counterpart in the CUDA library) ---- */
     int hydro_phi_level;               /* which phi the hydrodynamic update differentiates: 0 = phi^n (reading S16, what
                                           Algorithm 1's communication order implies), 1 = phi^{n+1}
@@ -273,10 +276,11 @@ static void guo_populations(const lattice *L, const double a[3], const double u[
  *   a~ = a - K^-1 S K (a - a_eq) + K^-1 (I - S/2) K F(avec, u)
  * computed as  r = S K (a - a_eq) - (K F - S K F / 2);  solve K y = r;  a~ = a - y. */
 static int collide_generic(const lattice *L, const rates *R, const double u[3], const double *a,
-                           const double *aeq, const double avec[3], double *out) {
+                           const double *aeq, const double avec[3], double *out, int raw_space) {
     double K[QMAX][QMAX], d[QMAX], Fi[QMAX], kd[QMAX] = {0}, kf[QMAX] = {0}, skd[QMAX], skf[QMAX], r[QMAX], y[QMAX];
     int Q = L->Q;
-    build_K(L, u, K);
+    const double rest[3] = {0.0, 0.0, 0.0};
+    build_K(L, raw_space ? rest : u, K); /* raw moments (MRT) = the same basis about the lattice at rest */
     guo_populations(L, avec, u, Fi);
     for (int i = 0; i < Q; i++) d[i] = a[i] - aeq[i];
     for (int m = 0; m < Q; m++) {
@@ -357,6 +361,7 @@ int tcpo_create(int nx, int ny, int nz, const tcpo_params *p, tcpo_sim **out) {
     }
     if (p->thermal < TCPO_LB_D3Q7 || p->thermal > TCPO_RK4) return fail(TCPO_EINVAL, "bad thermal variant");
     if (p->hydro_lattice != 27 && p->hydro_lattice != 19) return fail(TCPO_EINVAL, "hydro_lattice must be 27 or 19");
+    if (p->collision_space != 0 && p->collision_space != 1) return fail(TCPO_EINVAL, "collision_space must be 0 (central) or 1 (raw)");
     if (!(p->tau_H > -0.5) || !(p->tau_L > -0.5)) return fail(TCPO_EINVAL, "tau <= -1/2");
     if (!(p->M > 0) || !(p->xi > 0)) return fail(TCPO_EINVAL, "M, xi must be > 0");
     if (!(p->rho_H > 0) || !(p->rho_L > 0)) return fail(TCPO_EINVAL, "rho must be > 0");
@@ -588,7 +593,7 @@ static int update_h(tcpo_sim *s) {
                 double a[3] = {mag * G[0] / nrm, mag * G[1] / nrm, mag * G[2] / nrm};
                 double u[3] = {s->u[k], s->u[N + k], s->u[2 * N + k]};
                 eq_scalar(L, phin, u, heq); /* eq. 12 with phi' */
-                if (collide_generic(L, &R, u, hp, heq, a, hout)) bad |= 1;
+                if (collide_generic(L, &R, u, hp, heq, a, hout, P->collision_space)) bad |= 1;
                 for (int i = 0; i < 27; i++) s->h2[(size_t)i * N + k] = hout[i];
                 s->phi2[k] = phin;
             }
@@ -664,7 +669,7 @@ static int update_g(tcpo_sim *s) {
                 double om = 1.0 / (tau + 0.5);
                 rates R = {1.0, 1.0, om, P->s_bulk, P->s_high};
                 if (P->high_rate_equals_shear) { R.r0 = R.r1 = R.r2s = R.r2b = R.r3 = om; }
-                if (collide_generic(L, &R, u, gp, geq, a, gout)) bad |= 1;
+                if (collide_generic(L, &R, u, gp, geq, a, gout, P->collision_space)) bad |= 1;
                 for (int i = 0; i < L->Q; i++) s->g2[(size_t)i * N + k] = gout[i];
                 s->u[k] = u[0]; s->u[N + k] = u[1]; s->u[2 * N + k] = u[2]; /* u is only read locally */
             }
@@ -694,7 +699,7 @@ static int update_f(tcpo_sim *s) {
                 double u[3] = {s->u[k], s->u[N + k], s->u[2 * N + k]};
                 double zero[3] = {0, 0, 0};
                 eq_scalar(L, Tn, u, feq);
-                if (collide_generic(L, &R, u, fp, feq, zero, fout)) bad |= 1;
+                if (collide_generic(L, &R, u, fp, feq, zero, fout, P->collision_space)) bad |= 1;
                 double qT = s->q ? s->q[k] : 0.0;
                 for (int i = 0; i < L->Q; i++) s->f2[(size_t)i * N + k] = fout[i] + L->w[i] * qT; /* eq. 27 */
                 s->T2[k] = Tn;
@@ -828,6 +833,17 @@ int tcpo_lattice(int Q, int *c_out, double *w_out, int *opp_out, int *order_out)
 
 /* one generic collision on one cell.  kind: 0 scalar equilibrium (eq. 12) with moment s0,
  * 1 hydrodynamic equilibrium (eq. 18) with p* = s0.  rate5 = {r0, r1, r2s, r2b, r3}. */
+int tcpo_collide_cell_space(int Q, int kind, const double *rate5, const double *u, double s0, const double *avec,
+                            const double *a_in, double *a_out, int raw_space) {
+    lattice L;
+    if (lattice_build(&L, Q)) return fail(TCPO_EINVAL, "bad Q");
+    rates R = {rate5[0], rate5[1], rate5[2], rate5[3], rate5[4]};
+    double eq[QMAX];
+    if (kind == 0) eq_scalar(&L, s0, u, eq); else eq_hydro(&L, s0, u, eq);
+    if (collide_generic(&L, &R, u, a_in, eq, avec, a_out, raw_space)) return fail(TCPO_ESTATE, "singular K");
+    return TCPO_OK;
+}
+
 int tcpo_collide_cell(int Q, int kind, const double *rate5, const double *u, double s0, const double *avec,
                       const double *a_in, double *a_out) {
     lattice L;
@@ -835,7 +851,7 @@ int tcpo_collide_cell(int Q, int kind, const double *rate5, const double *u, dou
     rates R = {rate5[0], rate5[1], rate5[2], rate5[3], rate5[4]};
     double eq[QMAX];
     if (kind == 0) eq_scalar(&L, s0, u, eq); else eq_hydro(&L, s0, u, eq);
-    if (collide_generic(&L, &R, u, a_in, eq, avec, a_out)) return fail(TCPO_ESTATE, "singular K");
+    if (collide_generic(&L, &R, u, a_in, eq, avec, a_out, 0)) return fail(TCPO_ESTATE, "singular K");
     return TCPO_OK;
 }
 

@@ -34,6 +34,7 @@ class Params(C.Structure):
         ("sigma_TT", C.c_double),
         ("wall_contact_angle", (C.c_double * 2) * 3),   # degrees, reading S20
         ("hydro_lattice", C.c_int),        # 27 or 19
+        ("collision_space", C.c_int),      # 0 central moments, 1 raw moments (MRT)
         ("hydro_phi_level", C.c_int),      # oracle-only (reading S16): 0 = phi^n, 1 = phi^{n+1}
     ]
 
@@ -49,6 +50,7 @@ DEFAULTS = dict(
     sigma_TT=0.0,
     wall_contact_angle=((90.0, 90.0), (90.0, 90.0), (90.0, 90.0)),
     hydro_lattice=27,
+    collision_space=0,
     hydro_phi_level=0,
 )
 
@@ -78,6 +80,7 @@ def make_params(d: dict) -> Params:
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
     p.hydro_phi_level = int(v["hydro_phi_level"])
     p.hydro_lattice = int(v["hydro_lattice"])
+    p.collision_space = int(v["collision_space"])
     for a in range(3):
         for f in range(2):
             for c in range(3):
@@ -106,6 +109,7 @@ def lib():
         L.tcpo_read_populations.argtypes = [C.c_void_p, C.c_int, dp]
         L.tcpo_lattice.argtypes = [C.c_int, ip, dp, ip, ip]
         L.tcpo_collide_cell.argtypes = [C.c_int, C.c_int, dp, dp, C.c_double, dp, dp, dp]
+        L.tcpo_collide_cell_space.argtypes = [C.c_int, C.c_int, dp, dp, C.c_double, dp, dp, dp, C.c_int]
         L.tcpo_central_moment_matrix.argtypes = [C.c_int, dp, dp]
         L.tcpo_fd.argtypes = [C.c_void_p, dp, C.c_int, dp, dp]
         L.tcpo_last_error.restype = C.c_char_p
@@ -225,6 +229,13 @@ def collide_cell(Q, kind, rates5, u, s0, avec, a_in):
     rates5, u, avec, a_in = _f64(rates5), _f64(u), _f64(avec), _f64(a_in)
     out = np.empty(Q)
     _check(lib().tcpo_collide_cell(Q, kind, _dp(rates5), _dp(u), float(s0), _dp(avec), _dp(a_in), _dp(out)))
+    return out
+
+
+def collide_cell_space(Q, kind, rates5, u, s0, avec, a_in, raw_space):
+    rates5, u, avec, a_in = _f64(rates5), _f64(u), _f64(avec), _f64(a_in)
+    out = np.empty(Q)
+    _check(lib().tcpo_collide_cell_space(Q, kind, _dp(rates5), _dp(u), float(s0), _dp(avec), _dp(a_in), _dp(out), int(raw_space)))
     return out
 
 

@@ -36,7 +36,8 @@ enum { TCP_F64 = 0, TCP_F32 = 1 };
 enum { TCP_THERMAL_LB_D3Q7 = 0, TCP_THERMAL_LB_D3Q15, TCP_THERMAL_LB_D3Q19, TCP_THERMAL_LB_D3Q27,
        TCP_THERMAL_RK2, TCP_THERMAL_RK4 };
 enum { TCP_BC_PERIODIC = 0, TCP_BC_WALLS = 1 };
-enum { TCP_STREAM_TWO_GRID = 0, TCP_STREAM_AA = 1 }; /* AA: in place, one grid of populations (half the memory) */
+enum { TCP_STREAM_TWO_GRID = 0, TCP_STREAM_AA = 1 };
+enum { TCP_SPACE_CENTRAL = 0, TCP_SPACE_RAW = 1 };   /* collision space: central moments (the paper's model) or raw moments (MRT) */ /* AA: in place, one grid of populations (half the memory) */
 
 /* The paper's problem statement (sections 2.1-2.3).  Fill `struct_size = sizeof(tcp_params)`. */
 typedef struct tcp_params {
@@ -74,6 +75,10 @@ typedef struct tcp_params {
                                           often rely on a D3Q19 or D3Q27 stencil"; weights eq. B.3, central-moment
                                           basis x^a y^b z^c with a, b, c <= 2 and abc = 0).  19 moves 16 values per cell less
                                           (928 instead of 1056 B with the D3Q7 thermal LB); collisions: s_high = 1 or BGK only */
+    int collision_space;               /* TCP_SPACE_CENTRAL (default): moments about the local velocity; TCP_SPACE_RAW: the same
+                                          basis and rates about the lattice at rest, i.e. the multiple-relaxation-time (MRT) operator
+                                          ("the SRT or MRT methods retain widespread usage").  With
+                                          high_rate_equals_shear = 1 (SRT / BGK) the two coincide.  Same kernels, same cost */
 } tcp_params;
 
 /* Fill *p with the defaults: struct_size, fp64, thermal LB D3Q7, two-grid, periodic x 3, rho = 1, tau = 0.6, xi = 4,

@@ -80,7 +80,8 @@ def make_params(d: dict) -> Params:
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
     p.hydro_phi_level = int(v["hydro_phi_level"])
     p.hydro_lattice = int(v["hydro_lattice"])
-    p.collision_space = int(v["collision_space"])
+    cs = v["collision_space"]
+    p.collision_space = {"central": 0, "raw": 1}[cs] if isinstance(cs, str) else int(cs)
     for a in range(3):
         for f in range(2):
             for c in range(3):

@@ -17,6 +17,7 @@ PRECISION = {"f64": 0, "f32": 1}
 THERMAL = {"lb_d3q7": 0, "lb_d3q15": 1, "lb_d3q19": 2, "lb_d3q27": 3, "rk2": 4, "rk4": 5}
 BC = {"periodic": 0, "walls": 1}
 STREAMING = {"two_grid": 0, "aa": 1}
+SPACE = {"central": 0, "raw": 1}
 
 
 class tcp_params(C.Structure):
@@ -39,6 +40,7 @@ class tcp_params(C.Structure):
         ("sigma_TT", C.c_double),
         ("wall_contact_angle", (C.c_double * 2) * 3),
         ("hydro_lattice", C.c_int),
+        ("collision_space", C.c_int),
     ]
 
 
@@ -53,6 +55,7 @@ PARAM_DEFAULTS = dict(
     sigma_TT=0.0,
     wall_contact_angle=((90.0, 90.0), (90.0, 90.0), (90.0, 90.0)),
     hydro_lattice=27,
+    collision_space="central",
 )
 
 
@@ -79,6 +82,7 @@ def make_params(d: dict) -> tcp_params:
         setattr(p, k, float(v[k]))
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
     p.hydro_lattice = int(v["hydro_lattice"])
+    p.collision_space = enum(SPACE, v["collision_space"])
     for a in range(3):
         for f in range(2):
             for c in range(3):

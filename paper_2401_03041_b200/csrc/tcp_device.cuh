@@ -42,6 +42,7 @@ struct StepArgs {
     real wall_u[3][2][3];            // wall velocity [axis][face][component] (moving wall, reading S18)
     int wetting;                     // any wall with a contact angle other than 90 degrees
     real wet_a[3][2];                // a = -(2 / xi) cos(theta) of each wall (wetting boundary condition, reading S20); 0 = neutral
+    real cm_frame;                   // 1: central moments (about u); 0: raw moments (about the lattice at rest) = MRT (tcp_params::collision_space)
 };
 
 // packed pairs: the arrays are plain float arrays, the scalars are broadcast pairs
@@ -75,12 +76,13 @@ struct StepArgs<f32x2> {
     float wall_u[3][2][3];
     int wetting;
     float wet_a[3][2];
+    f32x2 cm_frame;
     __host__ explicit StepArgs(const StepArgs<float>& A)
         : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), cell0(A.cell0), cell1(A.cell1), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
           f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src), rk1_out(A.rk1_out), rk1_acc(A.rk1_acc), rk1_c_out(A.rk1_c_out), rk1_c_acc(A.rk1_c_acc),
           rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), inv_xi(A.inv_xi), sigma_ref(A.sigma_ref),
           sigma_T(A.sigma_T), T_ref(A.T_ref), sigma_TT(A.sigma_TT), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
-          s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving), wetting(A.wetting) {
+          s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving), wetting(A.wetting), cm_frame(A.cm_frame) {
         for (int k = 0; k < 3; ++k) { div_nx[k] = A.div_nx[k]; div_ny[k] = A.div_ny[k]; div_hx[k] = A.div_hx[k]; }
         for (int a = 0; a < 3; ++a) {
             wall[a] = A.wall[a];

@@ -127,8 +127,11 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
         const real m[3] = {k1 * ((M.mx - phin * un[0]) + real(0.5) * a[0]),
                            k1 * ((M.my - phin * un[1]) + real(0.5) * a[1]),
                            k1 * ((M.mz - phin * un[2]) + real(0.5) * a[2])};
+        // the populations that carry the relaxed moments: central moments about u, or, for the raw-moment (MRT) space, about
+        // the lattice at rest.  The relaxed amplitudes are the same in both spaces: (h - h_eq) + F/2 has no zeroth moment, so
+        // its first central and raw moments coincide
         R1D<real> rx, ry, rz;
-        rx.set(un[0]); ry.set(un[1]); rz.set(un[2]);
+        rx.set(A.cm_frame * un[0]); ry.set(A.cm_frame * un[1]); rz.set(A.cm_frame * un[2]);
         add_first_order27<real>(m, rx, ry, rz, out);
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = out[q];
@@ -214,7 +217,8 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
 #pragma unroll
             for (int q = 0; q < 27; ++q) X[q] = g[q] - X[q];
         }
-        central_transform27<real, true>(X, u);
+        const real uf[3] = {A.cm_frame * u[0], A.cm_frame * u[1], A.cm_frame * u[2]};   // raw-moment space: transform about rest
+        central_transform27<real, true>(X, uf);
         const real k2 = real(1) - om, k3 = real(1) - A.s_high;
         const real tr3 = (X[2] + X[6] + X[18]) * real(1.0 / 3.0), kb = (real(1) - A.s_bulk) * tr3;
 #pragma unroll
@@ -224,7 +228,7 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
             else if (order == 2) X[q] = (q == 2 || q == 6 || q == 18) ? k2 * (X[q] - tr3) + kb : k2 * X[q];
             else X[q] = k3 * X[q];
         }
-        central_transform27<real, false>(X, u);
+        central_transform27<real, false>(X, uf);
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = out[q] + X[q];
     } else {
@@ -240,12 +244,15 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
         const real tr3 = (kxx + kyy + kzz) * real(1.0 / 3.0);
         const real k2 = real(1) - om, kb = (real(1) - A.s_bulk) * tr3;
         kxx = k2 * (kxx - tr3) + kb; kyy = k2 * (kyy - tr3) + kb; kzz = k2 * (kzz - tr3) + kb;
+        // (g - g_eq) + F/2 has neither a zeroth nor a first moment, so its second central and raw moments coincide; only the
+        // populations that carry them differ between the central-moment and the raw-moment (MRT) space
+        const real uf[3] = {A.cm_frame * u[0], A.cm_frame * u[1], A.cm_frame * u[2]};
         if constexpr (QH == 27) {
             R1D<real> rx, ry, rz;
-            rx.set(u[0]); ry.set(u[1]); rz.set(u[2]);
+            rx.set(uf[0]); ry.set(uf[1]); rz.set(uf[2]);
             add_second_order27<real>(kxx, kyy, kzz, k2 * kxy, k2 * kxz, k2 * kyz, rx, ry, rz, out);
         } else {
-            add_second_order19<real>(kxx, kyy, kzz, k2 * kxy, k2 * kxz, k2 * kyz, u, out);
+            add_second_order19<real>(kxx, kyy, kzz, k2 * kxy, k2 * kxz, k2 * kyz, uf, out);
         }
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = out[q];
@@ -281,12 +288,13 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
     } else {
         const real k1 = real(1) - w;
         const real m[3] = {k1 * (j[0] - Tn * u[0]), k1 * (j[1] - Tn * u[1]), k1 * (j[2] - Tn * u[2])};
+        const real uf[3] = {A.cm_frame * u[0], A.cm_frame * u[1], A.cm_frame * u[2]};   // see collide_phase
         if constexpr (Q == 27) {
             R1D<real> rx, ry, rz;
-            rx.set(u[0]); ry.set(u[1]); rz.set(u[2]);
+            rx.set(uf[0]); ry.set(uf[1]); rz.set(uf[2]);
             add_first_order27<real>(m, rx, ry, rz, out);
         } else {
-            add_first_order_thermal<real, Q>(m, u, out);
+            add_first_order_thermal<real, Q>(m, uf, out);
         }
     }
     if constexpr (real_traits<real>::single) {   // see conserve_zeroth27

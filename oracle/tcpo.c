@@ -72,6 +72,10 @@ typedef struct tcpo_params {
     int collision_space;               /* 0 (default): central moments, K(u)_{m,i} = b_m(c_i - u); 1: raw moments, K(0) -- the
                                           multiple-relaxation-time (MRT) operator with the same basis and rates ("the SRT or MRT methods
                                           retain widespread usage") */
+    int equilibrium;                   /* 0 (default): the second-order equilibria printed in the paper (eqs. 12, 18); 1: the continuous
+                                          Maxwellian taken in central-moment space (D3Q27 lattices only): central moments of x^a y^b z^c
+                                          = s m_a m_b m_c with m_0 = 1, m_1 = 0, m_2 = c_s^2, in place of those of eq. 12; eq. 18
+                                          becomes w_i (p* - 1) + that equilibrium with s = 1 */
     /* ---- oracle-only switches (no counterpart in the CUDA library) ---- */
     int hydro_phi_level;               /* which phi the hydrodynamic update differentiates: 0 = phi^n (reading S16, what
                                           Algorithm 1's communication order implies), 1 = phi^{n+1}
@@ -260,6 +264,27 @@ static void eq_hydro(const lattice *L, double pstar, const double u[3], double *
     }
 }
 
+/* Maxwellian equilibrium in central-moment space (tcpo_params::equilibrium = 1), monomial bases only (D3Q27, D3Q19):
+ * the populations a with K(u) a = kappa^M, kappa^M of x^a y^b z^c = s m_a m_b m_c, m = (1, 0, c_s^2) -- the central
+ * moments of the continuous Maxwell-Boltzmann distribution of density s, velocity u, temperature c_s^2 on the basis. */
+static int eq_scalar_maxwell(const lattice *L, double s, const double u[3], double *out) {
+    static const double m1d[3] = {1.0, 0.0, CS2};
+    double K[QMAX][QMAX], kap[QMAX];
+    build_K(L, u, K);
+    for (int m = 0; m < L->Q; m++) {
+        if (L->nterm[m] != 1) return -1;
+        kap[m] = s * m1d[L->e[m][0][0]] * m1d[L->e[m][0][1]] * m1d[L->e[m][0][2]];
+    }
+    return solve_dense(L->Q, K, kap, out);
+}
+
+/* eq. 18 with the bracket [...] = f_eq(rho = 1, u) / w_i - 1 taken from the Maxwellian: w_i (p* - 1) + a^M(1, u) */
+static int eq_hydro_maxwell(const lattice *L, double pstar, const double u[3], double *out) {
+    if (eq_scalar_maxwell(L, 1.0, u, out)) return -1;
+    for (int i = 0; i < L->Q; i++) out[i] += L->w[i] * (pstar - 1.0);
+    return 0;
+}
+
 /* Guo force populations (ref. [20] named at PAPER.md:100, 118):
  *   F_i(a,u) = w_i [ (c_i - u)/c_s^2 + (c_i.u) c_i / c_s^4 ] . a */
 static void guo_populations(const lattice *L, const double a[3], const double u[3], double *out) {
@@ -361,6 +386,9 @@ int tcpo_create(int nx, int ny, int nz, const tcpo_params *p, tcpo_sim **out) {
     }
     if (p->thermal < TCPO_LB_D3Q7 || p->thermal > TCPO_RK4) return fail(TCPO_EINVAL, "bad thermal variant");
     if (p->hydro_lattice != 27 && p->hydro_lattice != 19) return fail(TCPO_EINVAL, "hydro_lattice must be 27 or 19");
+    if (p->equilibrium != 0 && p->equilibrium != 1) return fail(TCPO_EINVAL, "equilibrium must be 0 (printed second-order) or 1 (Maxwellian)");
+    if (p->equilibrium == 1 && (p->hydro_lattice != 27 || (p->thermal <= TCPO_LB_D3Q27 && p->thermal != TCPO_LB_D3Q27)))
+        return fail(TCPO_EUNSUPPORTED, "Maxwellian equilibrium: D3Q27 lattices only (hydro_lattice = 27; thermal D3Q27 LB or RK)");
     if (p->collision_space != 0 && p->collision_space != 1) return fail(TCPO_EINVAL, "collision_space must be 0 (central) or 1 (raw)");
     if (!(p->tau_H > -0.5) || !(p->tau_L > -0.5)) return fail(TCPO_EINVAL, "tau <= -1/2");
     if (!(p->M > 0) || !(p->xi > 0)) return fail(TCPO_EINVAL, "M, xi must be > 0");
@@ -432,11 +460,13 @@ int tcpo_init_fields(tcpo_sim *s, const double *phi, const double *u, const doub
     for (long k = 0; k < (long)N; k++) {
         double uu[3] = {s->u[k], s->u[N + k], s->u[2 * N + k]};
         double e[QMAX];
-        eq_scalar(&s->L27, s->phi[k], uu, e);
+        const int mx = s->P.equilibrium == 1;
+        if (mx) eq_scalar_maxwell(&s->L27, s->phi[k], uu, e); else eq_scalar(&s->L27, s->phi[k], uu, e);
         for (int i = 0; i < 27; i++) s->h[i * N + k] = e[i];
-        eq_hydro(&s->LH, 0.0, uu, e);
+        if (mx) eq_hydro_maxwell(&s->LH, 0.0, uu, e); else eq_hydro(&s->LH, 0.0, uu, e);
         for (int i = 0; i < s->LH.Q; i++) s->g[i * N + k] = e[i];
         if (s->thermal_is_lb) {
+            if (mx) eq_scalar_maxwell(&s->LT, s->T[k], uu, e); else
             eq_scalar(&s->LT, s->T[k], uu, e);
             for (int i = 0; i < s->LT.Q; i++) s->f[i * N + k] = e[i];
         }
@@ -592,7 +622,8 @@ static int update_h(tcpo_sim *s) {
                 double mag = CS2 * (4.0 * ph * (1.0 - ph) / P->xi);
                 double a[3] = {mag * G[0] / nrm, mag * G[1] / nrm, mag * G[2] / nrm};
                 double u[3] = {s->u[k], s->u[N + k], s->u[2 * N + k]};
-                eq_scalar(L, phin, u, heq); /* eq. 12 with phi' */
+                if (P->equilibrium == 1) { if (eq_scalar_maxwell(L, phin, u, heq)) bad |= 1; }
+                else eq_scalar(L, phin, u, heq); /* eq. 12 with phi' */
                 if (collide_generic(L, &R, u, hp, heq, a, hout, P->collision_space)) bad |= 1;
                 for (int i = 0; i < 27; i++) s->h2[(size_t)i * N + k] = hout[i];
                 s->phi2[k] = phin;
@@ -652,7 +683,8 @@ static int update_g(tcpo_sim *s) {
                     ustar[al] = j[al] + F0[al] / (2.0 * rho); /* predictor, S4 */
                 }
                 /* non-equilibrium second moments about g_eq(p*, u*) and eq. 21 */
-                eq_hydro(L, pstar, ustar, geq);
+                if (P->equilibrium == 1) { if (eq_hydro_maxwell(L, pstar, ustar, geq)) bad |= 1; }
+                else eq_hydro(L, pstar, ustar, geq);
                 double Pi[3][3] = {{0}};
                 for (int i = 0; i < L->Q; i++)
                     for (int al = 0; al < 3; al++)
@@ -665,7 +697,8 @@ static int update_g(tcpo_sim *s) {
                     u[al] = j[al] + F[al] / (2.0 * rho); /* O7, S6 */
                     a[al] = F[al] / rho;
                 }
-                eq_hydro(L, pstar, u, geq); /* eq. 18 */
+                if (P->equilibrium == 1) { if (eq_hydro_maxwell(L, pstar, u, geq)) bad |= 1; }
+                else eq_hydro(L, pstar, u, geq); /* eq. 18 */
                 double om = 1.0 / (tau + 0.5);
                 rates R = {1.0, 1.0, om, P->s_bulk, P->s_high};
                 if (P->high_rate_equals_shear) { R.r0 = R.r1 = R.r2s = R.r2b = R.r3 = om; }
@@ -698,7 +731,8 @@ static int update_f(tcpo_sim *s) {
                 if (P->high_rate_equals_shear) { R.r0 = R.r1 = R.r2s = R.r2b = R.r3 = w_T; }
                 double u[3] = {s->u[k], s->u[N + k], s->u[2 * N + k]};
                 double zero[3] = {0, 0, 0};
-                eq_scalar(L, Tn, u, feq);
+                if (P->equilibrium == 1) { if (eq_scalar_maxwell(L, Tn, u, feq)) bad |= 1; }
+                else eq_scalar(L, Tn, u, feq);
                 if (collide_generic(L, &R, u, fp, feq, zero, fout, P->collision_space)) bad |= 1;
                 double qT = s->q ? s->q[k] : 0.0;
                 for (int i = 0; i < L->Q; i++) s->f2[(size_t)i * N + k] = fout[i] + L->w[i] * qT; /* eq. 27 */

@@ -35,6 +35,7 @@ class Params(C.Structure):
         ("wall_contact_angle", (C.c_double * 2) * 3),   # degrees, reading S20
         ("hydro_lattice", C.c_int),        # 27 or 19
         ("collision_space", C.c_int),      # 0 central moments, 1 raw moments (MRT)
+        ("equilibrium", C.c_int),          # 0 printed second-order (eqs. 12, 18), 1 Maxwellian in central-moment space
         ("hydro_phi_level", C.c_int),      # oracle-only (reading S16): 0 = phi^n, 1 = phi^{n+1}
     ]
 
@@ -50,6 +51,7 @@ DEFAULTS = dict(
     sigma_TT=0.0,
     wall_contact_angle=((90.0, 90.0), (90.0, 90.0), (90.0, 90.0)),
     hydro_lattice=27,
+    equilibrium=0,
     collision_space=0,
     hydro_phi_level=0,
 )
@@ -80,6 +82,8 @@ def make_params(d: dict) -> Params:
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
     p.hydro_phi_level = int(v["hydro_phi_level"])
     p.hydro_lattice = int(v["hydro_lattice"])
+    eqm = v["equilibrium"]
+    p.equilibrium = {"second_order": 0, "maxwellian": 1}[eqm] if isinstance(eqm, str) else int(eqm)
     cs = v["collision_space"]
     p.collision_space = {"central": 0, "raw": 1}[cs] if isinstance(cs, str) else int(cs)
     for a in range(3):

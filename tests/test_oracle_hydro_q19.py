@@ -23,11 +23,11 @@ def test_weights_and_basis_of_the_q19_hydrodynamic_lattice():
 
 def test_poiseuille_profile_on_q19():
     """Single phase, body force, halfway bounce-back: u = g_x y (H - y) / (2 nu), nu = tau c_s^2 (A13, S6)."""
-    ny, nu, gx = 24, 0.2, 1e-6
+    ny, nu, gx = 20, 0.2, 1e-6
     o = tcpo.Oracle(1, ny, 1, dict(bc=("periodic", "walls", "periodic"), tau_H=3 * nu, tau_L=3 * nu, gravity=(gx, 0, 0),
                                    xi=1e30, hydro_lattice=19))
     o.init_fields(np.zeros((1, ny, 1)))
-    o.step(9000)
+    o.step(6000)
     phi, u, p, T = o.read_fields()
     o.close()
     yy = np.arange(ny) + 0.5

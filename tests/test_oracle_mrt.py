@@ -67,11 +67,11 @@ def test_raw_moment_balance(Q):
 
 def test_poiseuille_and_heat_decay_in_raw_moment_space():
     """The physical rates are the same in both spaces: nu = tau c_s^2 (Poiseuille, A13) and kappa (heat sinusoid, G4)."""
-    ny, nu, gx = 24, 0.2, 1e-6
+    ny, nu, gx = 20, 0.2, 1e-6
     o = tcpo.Oracle(1, ny, 1, dict(bc=("periodic", "walls", "periodic"), tau_H=3 * nu, tau_L=3 * nu, gravity=(gx, 0, 0),
                                    xi=1e30, collision_space=1))
     o.init_fields(np.zeros((1, ny, 1)))
-    o.step(9000)
+    o.step(6000)
     u = o.read_fields()[1]
     o.close()
     yy = np.arange(ny) + 0.5

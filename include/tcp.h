@@ -37,7 +37,8 @@ enum { TCP_THERMAL_LB_D3Q7 = 0, TCP_THERMAL_LB_D3Q15, TCP_THERMAL_LB_D3Q19, TCP_
        TCP_THERMAL_RK2, TCP_THERMAL_RK4 };
 enum { TCP_BC_PERIODIC = 0, TCP_BC_WALLS = 1 };
 enum { TCP_STREAM_TWO_GRID = 0, TCP_STREAM_AA = 1 };
-enum { TCP_SPACE_CENTRAL = 0, TCP_SPACE_RAW = 1 };   /* collision space: central moments (the paper's model) or raw moments (MRT) */ /* AA: in place, one grid of populations (half the memory) */
+enum { TCP_SPACE_CENTRAL = 0, TCP_SPACE_RAW = 1 };
+enum { TCP_EQ_SECOND_ORDER = 0, TCP_EQ_MAXWELLIAN = 1 };   /* equilibria: eqs. 12 / 18 as printed, or the Maxwellian in central-moment space */   /* collision space: central moments (the paper's model) or raw moments (MRT) */ /* AA: in place, one grid of populations (half the memory) */
 
 /* The paper's problem statement (sections 2.1-2.3).  Fill `struct_size = sizeof(tcp_params)`. */
 typedef struct tcp_params {
@@ -79,6 +80,11 @@ typedef struct tcp_params {
                                           basis and rates about the lattice at rest, i.e. the multiple-relaxation-time (MRT) operator
                                           ("the SRT or MRT methods retain widespread usage").  With
                                           high_rate_equals_shear = 1 (SRT / BGK) the two coincide.  Same kernels, same cost */
+    int equilibrium;                   /* TCP_EQ_SECOND_ORDER (default): eqs. 12 and 18 as printed; TCP_EQ_MAXWELLIAN: the continuous
+                                          Maxwell-Boltzmann distribution taken in central-moment space (central moments of x^a y^b z^c
+                                          = s m_a m_b m_c, m = (1, 0, c_s^2); on D3Q27 the product form), in place of eq. 12; eq. 18
+                                          becomes w_i (p* - 1) + that equilibrium with s = 1.  Moments up to second order are
+                                          unchanged.  D3Q27 lattices only: hydro_lattice = 27 and thermal D3Q27 LB / RK2 / RK4 */
 } tcp_params;
 
 /* Fill *p with the defaults: struct_size, fp64, thermal LB D3Q7, two-grid, periodic x 3, rho = 1, tau = 0.6, xi = 4,

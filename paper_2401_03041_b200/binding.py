@@ -18,6 +18,7 @@ THERMAL = {"lb_d3q7": 0, "lb_d3q15": 1, "lb_d3q19": 2, "lb_d3q27": 3, "rk2": 4, 
 BC = {"periodic": 0, "walls": 1}
 STREAMING = {"two_grid": 0, "aa": 1}
 SPACE = {"central": 0, "raw": 1}
+EQUILIBRIUM = {"second_order": 0, "maxwellian": 1}
 
 
 class tcp_params(C.Structure):
@@ -41,6 +42,7 @@ class tcp_params(C.Structure):
         ("wall_contact_angle", (C.c_double * 2) * 3),
         ("hydro_lattice", C.c_int),
         ("collision_space", C.c_int),
+        ("equilibrium", C.c_int),
     ]
 
 
@@ -56,6 +58,7 @@ PARAM_DEFAULTS = dict(
     wall_contact_angle=((90.0, 90.0), (90.0, 90.0), (90.0, 90.0)),
     hydro_lattice=27,
     collision_space="central",
+    equilibrium="second_order",
 )
 
 
@@ -83,6 +86,7 @@ def make_params(d: dict) -> tcp_params:
     p.high_rate_equals_shear = int(v["high_rate_equals_shear"])
     p.hydro_lattice = int(v["hydro_lattice"])
     p.collision_space = enum(SPACE, v["collision_space"])
+    p.equilibrium = enum(EQUILIBRIUM, v["equilibrium"])
     for a in range(3):
         for f in range(2):
             for c in range(3):

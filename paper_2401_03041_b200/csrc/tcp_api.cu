@@ -75,6 +75,12 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
         for (int fc = 0; fc < 2; ++fc)
             if (!(p->wall_contact_angle[a][fc] >= 0.0 && p->wall_contact_angle[a][fc] <= 180.0))
                 return fail(TCP_EINVAL, "wall_contact_angle must lie in [0, 180] degrees (default 90, see tcp_params_default)");
+    if (p->equilibrium != TCP_EQ_SECOND_ORDER && p->equilibrium != TCP_EQ_MAXWELLIAN) return fail(TCP_EINVAL, "equilibrium must be TCP_EQ_SECOND_ORDER or TCP_EQ_MAXWELLIAN");
+    if (p->equilibrium == TCP_EQ_MAXWELLIAN) {
+        const int qt = thermal_q(p->thermal);
+        if (p->hydro_lattice != 27 || (qt != 0 && qt != 27))
+            return fail(TCP_EUNSUPPORTED, "Maxwellian equilibrium: D3Q27 lattices only (hydro_lattice = 27; thermal D3Q27 LB, RK2 or RK4)");
+    }
     if (p->collision_space != TCP_SPACE_CENTRAL && p->collision_space != TCP_SPACE_RAW) return fail(TCP_EINVAL, "collision_space must be TCP_SPACE_CENTRAL or TCP_SPACE_RAW");
     if (p->hydro_lattice != 27 && p->hydro_lattice != 19) return fail(TCP_EINVAL, "hydro_lattice must be 27 or 19 (default 27, see tcp_params_default)");
     if (p->hydro_lattice == 19 && p->s_high != 1.0 && !p->high_rate_equals_shear)
@@ -208,6 +214,8 @@ tcp::StepArgs<real> make_args(const tcp_sim* s) {
                 if (P.wall_u[a][fc][k] != 0.0) A.moving = 1;
             }
     A.cm_frame = (real)(P.collision_space == TCP_SPACE_RAW ? 0.0 : 1.0);
+    A.maxwell = P.equilibrium == TCP_EQ_MAXWELLIAN;
+    A.eq_sigma = (real)(A.maxwell ? 0.0 : 1.0);
     // wetting (reading S20): a = -(2 / xi) cos(theta) per wall; exactly 0 for the neutral 90 degrees
     A.wetting = 0;
     for (int a = 0; a < 3; ++a)

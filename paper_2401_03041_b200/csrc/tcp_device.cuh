@@ -42,6 +42,8 @@ struct StepArgs {
     real wall_u[3][2][3];            // wall velocity [axis][face][component] (moving wall, reading S18)
     int wetting;                     // any wall with a contact angle other than 90 degrees
     real wet_a[3][2];                // a = -(2 / xi) cos(theta) of each wall (wetting boundary condition, reading S20); 0 = neutral
+    int maxwell;                     // 1: Maxwellian (product-form) equilibria instead of the printed second-order ones (tcp_params::equilibrium)
+    real eq_sigma;                   // 1 - maxwell: weight of the second-order polynomial equilibrium inside E (equilibrium_plus_half_force27)
     real cm_frame;                   // 1: central moments (about u); 0: raw moments (about the lattice at rest) = MRT (tcp_params::collision_space)
 };
 
@@ -76,13 +78,14 @@ struct StepArgs<f32x2> {
     float wall_u[3][2][3];
     int wetting;
     float wet_a[3][2];
-    f32x2 cm_frame;
+    int maxwell;
+    f32x2 eq_sigma, cm_frame;
     __host__ explicit StepArgs(const StepArgs<float>& A)
         : nx(A.nx), ny(A.ny), nz(A.nz), ncell(A.ncell), cell0(A.cell0), cell1(A.cell1), aa(A.aa), h_in(A.h_in), h_out(A.h_out), g_in(A.g_in), g_out(A.g_out),
           f_in(A.f_in), f_out(A.f_out), phi_in(A.phi_in), phi_out(A.phi_out), T_in(A.T_in), T_out(A.T_out), u(A.u), q_src(A.q_src), rk1_out(A.rk1_out), rk1_acc(A.rk1_acc), rk1_c_out(A.rk1_c_out), rk1_c_acc(A.rk1_c_acc),
           rho_L(A.rho_L), drho(A.drho), tau_L(A.tau_L), dtau(A.dtau), xi(A.xi), w_phi(A.w_phi), inv_xi(A.inv_xi), sigma_ref(A.sigma_ref),
           sigma_T(A.sigma_T), T_ref(A.T_ref), sigma_TT(A.sigma_TT), kappa_L(A.kappa_L), dkappa(A.dkappa), cp_L(A.cp_L), dcp(A.dcp),
-          s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving), wetting(A.wetting), cm_frame(A.cm_frame) {
+          s_bulk(A.s_bulk), s_high(A.s_high), eps(A.eps), moving(A.moving), wetting(A.wetting), maxwell(A.maxwell), eq_sigma(A.eq_sigma), cm_frame(A.cm_frame) {
         for (int k = 0; k < 3; ++k) { div_nx[k] = A.div_nx[k]; div_ny[k] = A.div_ny[k]; div_hx[k] = A.div_hx[k]; }
         for (int a = 0; a < 3; ++a) {
             wall[a] = A.wall[a];
@@ -363,6 +366,43 @@ __device__ __forceinline__ void equilibrium_plus_half_force27(real A0, const rea
         out[26 - q] = sym - asym;
     }
     out[13] = real(weight(Q, 0)) * A0;
+}
+
+// Maxwellian equilibrium (tcp_params::equilibrium = TCP_EQ_MAXWELLIAN): the continuous Maxwell-Boltzmann distribution in
+// central-moment space on D3Q27 is the product form  s prod_axis p(c_a; u_a),  p(0; u) = 2/3 - u^2 = w(0) (1 - 3/2 u^2),
+// p(+-1; u) = 1/6 +- u/2 + u^2/2 = w(1) (1 +- 3 u + 3 u^2)  (central moments 1, 0, 1/3 per axis).  Its moments up to second
+// order are those of the printed equilibria (eqs. 12, 18), so the relaxed moments of the closed-form collisions do not
+// change; only these populations replace the polynomial ones.   out_q += s w_q pi_x pi_y pi_z.
+// DEV: out_q += s w_q (pi_x pi_y pi_z - 1) -- the form the hydrodynamic populations need (eq. 18 subtracts w_q), evaluated
+// without ever forming the 1: with pi = 1 + d, d(0) = -3/2 u^2, d(+-1) = +-3u + 3u^2,
+//   pi_x pi_y - 1 = d_x + d_y + d_x d_y =: t,   pi_x pi_y pi_z - 1 = t + d_z + t d_z,
+// so that g~ stays a deviation of size O(u) also in single precision (w_q (p* - 1) + product would cancel to ~1e-4 relative).
+template <typename real, bool DEV>
+__device__ __forceinline__ void add_product_form27(real s, const real u[3], real out[27]) {
+    real d[3][3];   // [axis][c + 1]
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const real uu3 = real(3) * u[a] * u[a], u3 = real(3) * u[a];
+        d[a][1] = real(-0.5) * uu3;
+        d[a][0] = uu3 - u3;
+        d[a][2] = uu3 + u3;
+    }
+    real t[3][3];   // [cy][cx]: pi_x pi_y - 1
+#pragma unroll
+    for (int y = 0; y < 3; ++y)
+#pragma unroll
+        for (int x = 0; x < 3; ++x) t[y][x] = (d[0][x] + d[1][y]) + d[0][x] * d[1][y];
+#pragma unroll
+    for (int z = 0; z < 3; ++z)
+#pragma unroll
+        for (int y = 0; y < 3; ++y)
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {
+                const int q = 9 * z + 3 * y + x;
+                const real dev = (t[y][x] + d[2][z]) + t[y][x] * d[2][z];
+                const real sw = s * real(weight(27, cls27(q)));
+                out[q] += DEV ? sw * dev : sw + sw * dev;
+            }
 }
 
 // out_q += sum_alpha m_alpha R^alpha_q(u): populations whose first-order central moments are m and

@@ -114,10 +114,13 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
     }
     real b[3], v[3];
 #pragma unroll
-    for (int al = 0; al < 3; ++al) { b[al] = phin * un[al] + a[al]; v[al] = phin * un[al] + real(0.5) * a[al]; }
-    const real A0 = phin - real(1.5) * (un[0] * b[0] + un[1] * b[1] + un[2] * b[2]);
+    // E = sigma h_eq(eq. 12) + F/2; sigma = 1, or 0 with the Maxwellian equilibrium, whose product form is added instead
+    const real se = A.eq_sigma * phin;
+    for (int al = 0; al < 3; ++al) { b[al] = se * un[al] + a[al]; v[al] = se * un[al] + real(0.5) * a[al]; }
+    const real A0 = se - real(1.5) * (un[0] * b[0] + un[1] * b[1] + un[2] * b[2]);
     real out[27];
     equilibrium_plus_half_force27<real>(A0, un, v, b, out);
+    if (A.maxwell) add_product_form27<real, false>(phin, un, out);
     if (MODE == 1) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = (real(1) - w) * h[q] + w * out[q];
@@ -196,10 +199,22 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
     }
     real b[3], v[3];
 #pragma unroll
-    for (int al = 0; al < 3; ++al) { b[al] = u[al] + a[al]; v[al] = u[al] + real(0.5) * a[al]; }
+    // E = w_q p* + sigma w_q [poly(u) of eq. 18] + F/2; Maxwellian (sigma = 0): + w_q (pi_x pi_y pi_z - 1) instead of w_q poly(u)
+    const real sg = A.eq_sigma;
+    for (int al = 0; al < 3; ++al) { b[al] = sg * u[al] + a[al]; v[al] = sg * u[al] + real(0.5) * a[al]; }
     const real A0 = ps - real(1.5) * (u[0] * b[0] + u[1] * b[1] + u[2] * b[2]);
     real out[27];
     equilibrium_plus_half_force27<real, QH>(A0, u, v, b, out);
+    real pf[(MODE == 2) ? 27 : 1];           // general-rate mode: the product form is needed twice (in E(a) and in E(-a))
+    if constexpr (MODE == 2) {
+#pragma unroll
+        for (int q = 0; q < 27; ++q) pf[q] = real(0);
+        if (A.maxwell) add_product_form27<real, true>(real(1), u, pf);
+#pragma unroll
+        for (int q = 0; q < 27; ++q) out[q] += pf[q];
+    } else {
+        if (A.maxwell) add_product_form27<real, true>(real(1), u, out);
+    }
     if (MODE == 1) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = (real(1) - om) * g[q] + om * out[q];
@@ -212,10 +227,10 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
         {
             real bm[3], vm[3];
 #pragma unroll
-            for (int al = 0; al < 3; ++al) { bm[al] = u[al] - a[al]; vm[al] = u[al] - real(0.5) * a[al]; }
+            for (int al = 0; al < 3; ++al) { bm[al] = sg * u[al] - a[al]; vm[al] = sg * u[al] - real(0.5) * a[al]; }
             equilibrium_plus_half_force27<real, QH>(ps - real(1.5) * (u[0] * bm[0] + u[1] * bm[1] + u[2] * bm[2]), u, vm, bm, X);
 #pragma unroll
-            for (int q = 0; q < 27; ++q) X[q] = g[q] - X[q];
+            for (int q = 0; q < 27; ++q) X[q] = g[q] - (X[q] + pf[q]);
         }
         const real uf[3] = {A.cm_frame * u[0], A.cm_frame * u[1], A.cm_frame * u[2]};   // raw-moment space: transform about rest
         central_transform27<real, true>(X, uf);
@@ -282,7 +297,13 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
     const real kap = A.kappa_L + phi_new * A.dkappa;         // eq. 23 (G5)
     const real w = real(1) / (real(0.5) + real(3) * kap);    // eq. 29 read as a rate (G4)
     real out[Q];
-    thermal_equilibrium<real, Q>(Tn, u, out);
+    if constexpr (Q == 27) {
+        if (A.maxwell) {
+#pragma unroll
+            for (int q = 0; q < 27; ++q) out[q] = real(0);
+            add_product_form27<real, false>(Tn, u, out);
+        } else thermal_equilibrium<real, Q>(Tn, u, out);
+    } else thermal_equilibrium<real, Q>(Tn, u, out);
     if (MODE == 1) {
         static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; out[k] = (real(1) - w) * f[k] + w * out[k]; });
     } else {
@@ -711,12 +732,19 @@ __global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
     real out[27];
     {
         const real s = A.phi_in[cell];
-        const real su[3] = {s * u[0], s * u[1], s * u[2]};
-        equilibrium_plus_half_force27<real>(s - real(1.5) * s * uu, u, su, su, out);      // eq. 12
+        const real se = A.eq_sigma * s;
+        const real su[3] = {se * u[0], se * u[1], se * u[2]};
+        equilibrium_plus_half_force27<real>(se - real(1.5) * se * uu, u, su, su, out);    // eq. 12
+        if (A.maxwell) add_product_form27<real, false>(s, u, out);                       // or the Maxwellian
 #pragma unroll
         for (int q = 0; q < 27; ++q) { bool wl; *dst_of(A.h_out, 27, q, q, wl) = out[q]; }
     }
-    equilibrium_plus_half_force27<real, QH>(-real(1.5) * uu, u, u, u, out);               // eq. 18, p* = 0
+    {
+        const real sg = A.eq_sigma;
+        const real su[3] = {sg * u[0], sg * u[1], sg * u[2]};
+        equilibrium_plus_half_force27<real, QH>(-real(1.5) * sg * uu, u, su, su, out);                     // eq. 18, p* = 0
+        if (A.maxwell) add_product_form27<real, true>(real(1), u, out);                                   // or w (p* - 1) + Maxwellian
+    }
     static_for<0, QH>([&](auto K) {
         constexpr int k = decltype(K)::value, q = q_of(QH, k);
         bool wl;
@@ -726,6 +754,13 @@ __global__ void __launch_bounds__(kBlock) init_kernel(const StepArgs<real> A) {
     if constexpr (QT > 0) {
         real f[QT];
         thermal_equilibrium<real, QT>(A.T_in[cell], u, f);
+        if constexpr (QT == 27) {
+            if (A.maxwell) {
+#pragma unroll
+                for (int q = 0; q < 27; ++q) f[q] = real(0);
+                add_product_form27<real, false>(A.T_in[cell], u, f);
+            }
+        }
         static_for<0, QT>([&](auto K) {
             constexpr int k = decltype(K)::value, q = q_of(QT, k);
             bool wl;

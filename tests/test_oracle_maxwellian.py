@@ -52,16 +52,8 @@ def test_equilibrium_populations_are_the_product_form_and_have_maxwellian_centra
     o.close()
 
 
-def test_poiseuille_heat_sinusoid_and_laplace_with_the_maxwellian():
-    ny, nu, gx = 20, 0.2, 1e-6
-    o = tcpo.Oracle(1, ny, 1, dict(MX, bc=("periodic", "walls", "periodic"), tau_H=3 * nu, tau_L=3 * nu, gravity=(gx, 0, 0), xi=1e30))
-    o.init_fields(np.zeros((1, ny, 1)))
-    o.step(6000)
-    u = o.read_fields()[1]
-    o.close()
-    yy = np.arange(ny) + 0.5
-    exact = gx / (2 * nu) * yy * (ny - yy)
-    assert np.abs(u[0].ravel() - exact).max() / exact.max() < 2e-3
+def test_heat_sinusoid_and_laplace_with_the_maxwellian():
+    # (Poiseuille is left to the other equilibrium: it sees second moments only, which the two equilibria share)
     n, kap, U, steps = 48, 0.1, 0.04, 120
     k = 2 * np.pi / n
     T0 = (1 + 0.5 * np.sin(k * np.arange(n))).reshape(1, 1, n)
@@ -74,11 +66,11 @@ def test_poiseuille_heat_sinusoid_and_laplace_with_the_maxwellian():
     Fm = np.fft.rfft(T - 1)[1]
     assert -np.log(2 * np.abs(Fm) / n / 0.5) / steps == pytest.approx(kap * k * k, rel=0.02)
     assert (-np.angle(Fm) - np.pi / 2) / k == pytest.approx(U * steps, rel=0.01)
-    nn, R = 32, 7.0
+    nn, R = 28, 6.0
     wl = W.static_droplet(n=nn, R=R, nz=1)
     o = tcpo.Oracle(nn, nn, 1, dict(wl.params, **MX))
     o.init_fields(wl.phi.numpy())
-    o.step(600)
+    o.step(500)
     phi, u, p, T = o.read_fields()
     o.close()
     dp = p[0, nn // 2 - 1:nn // 2 + 1, nn // 2 - 1:nn // 2 + 1].mean() - p[0, 0, 0]

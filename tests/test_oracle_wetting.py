@@ -85,7 +85,7 @@ def _cap_angle(phi):
     return 2 * np.degrees(np.arctan(H / (0.5 * base)))
 
 
-@pytest.mark.parametrize("theta,steps", [(60.0, 1600), (120.0, 1000)])
+@pytest.mark.parametrize("theta,steps", [(60.0, 1200), (120.0, 1000)])
 def test_sessile_droplet_relaxes_to_the_prescribed_contact_angle(theta, steps):
     nx, ny, R, xi = 46, 18, 8.0, 4.0
     x = np.arange(nx)[None, :]; Y = np.arange(ny)[:, None] + 0.5
@@ -98,6 +98,6 @@ def test_sessile_droplet_relaxes_to_the_prescribed_contact_angle(theta, steps):
     o.step(steps)
     phi, u, _, _ = o.read_fields()
     o.close()
-    assert _cap_angle(phi[0]) == pytest.approx(theta, abs=3.0)       # measured 59.9 / 117.6 at these step counts
+    assert _cap_angle(phi[0]) == pytest.approx(theta, abs=3.0)       # measured 61.3 / 117.6 at these step counts; 59.2 / 118.3 after 3000
     assert abs(phi.sum() - phi0.sum()) / phi0.sum() < 1e-12
     assert np.abs(u).max() < 1e-3                                      # settling, not flying apart

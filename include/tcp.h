@@ -99,7 +99,7 @@ int tcp_params_default(tcp_params *p);
 int tcp_workspace_bytes(int nx, int ny, int nz, const tcp_params *p, size_t *bytes);
 
 /* Create a simulation; the library allocates the workspace (cudaMalloc) and a stream.
- * Validation: n >= 1 (>= 2 on WALLS axes), tau > -1/2, M, xi, rho, kappa, cp, eps_normal > 0, 0 < s_bulk, s_high < 2.
+ * Validation: n >= 1 (>= 2 on WALLS axes), nx*ny*nz <= 429 496 729 (32-bit offsets within a group of 9 population planes), tau > -1/2, M, xi, rho, kappa, cp, eps_normal > 0, 0 < s_bulk, s_high < 2.
  * The simulation lives on the CUDA device that is current at the call; every later call makes that device current
  * for its own duration, so simulations on several GPUs can be driven from one thread.
  * Errors: TCP_EINVAL, TCP_EUNSUPPORTED, TCP_ENOMEM, TCP_ECUDA. */

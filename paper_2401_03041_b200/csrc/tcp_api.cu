@@ -53,7 +53,8 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
     if (!p) return fail(TCP_EINVAL, "params is NULL");
     if (p->struct_size != sizeof(tcp_params)) return fail(TCP_EINVAL, "tcp_params.struct_size != sizeof(tcp_params)");
     if (nx < 1 || ny < 1 || nz < 1) return fail(TCP_EINVAL, "extents must be >= 1");
-    if ((double)nx * ny * nz >= 2147483647.0) return fail(TCP_EINVAL, "nx*ny*nz must be < 2^31");
+    // cell indices are 32-bit, and so is the offset of a population from the base of its group of 9 planes (tcp_step.cuh): 10 N < 2^32
+    if ((double)nx * ny * nz > 429496729.0) return fail(TCP_EINVAL, "nx*ny*nz must be <= 429 496 729 (10 nx ny nz < 2^32)");
     if (ny > 65535 * 8 || nz > 65535) return fail(TCP_EINVAL, "ny must be <= 524280 and nz <= 65535 (grid limits)");
     const int n[3] = {nx, ny, nz};
     for (int a = 0; a < 3; ++a) {

@@ -139,6 +139,9 @@ __device__ __forceinline__ void stencil27_pair(const StepArgs<f32x2>& A, const N
 // the shared memory (as in the fp64 D3Q15 / D3Q19 kernels, tcp_step.cuh): 512^3 D3Q15 16.70 -> 16.03 ms, D3Q19 17.29 -> 16.42,
 // D3Q27 18.55 -> 18.35, D3Q7 (three blocks either way) 14.34 -> 14.02 sustained; the RK paths (Q_T = 0) lose 0.5-1 % and keep h
 // staged
+#ifndef TCP_PAIR_ADDR32
+#define TCP_PAIR_ADDR32 TCP_ADDR32
+#endif
 #ifndef TCP_PAIR_HDIRECT
 #define TCP_PAIR_HDIRECT 1
 #endif
@@ -161,15 +164,32 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
     const int cell = nb.idx;
     constexpr int aa = AA;
 
+    // element (plane, off) of a population array with a 32-bit offset from the uniform base of its group of 9 planes
+    // (fused_step_async_kernel, tcp_step.cuh)
+    const unsigned Nu = (unsigned)A.ncell;
+    // (only where h is staged too: with h pulled into registers the variants lose -- 512^3 sustained D3Q7 13.48 vs 12.67 ms,
+    // D3Q19 15.88 vs 15.30, more spills -- while RK2 gains, 12.10 vs 12.46-12.50, and AA is unchanged)
+    constexpr bool A32 = TCP_PAIR_ADDR32 && !pair_h_direct<QT, AA>();
+    auto elem = [&](auto* base, int plane, int off) {
+        if constexpr (A32) {
+            const int g = plane / 9;
+            auto* gb = base + (long long)(9 * g) * N;
+            asm("" : "+l"(gb));
+            __builtin_assume(__isGlobal(gb));
+            return gb + (unsigned)((unsigned)(plane - 9 * g) * Nu + (unsigned)off);
+        } else {
+            return base + plane * N + off;
+        }
+    };
     // issue the pulls of both cells of direction (Q, k, q27) into the slot (addressing table: fused_step_async_kernel)
     auto issue = [&](float2* slot, const float* base, int Q, int k, int q27i) {
         const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
-        if (aa == 1) { cp_async_8(slot, base + k * N + cell); return; }
+        if (aa == 1) { cp_async_8(slot, elem(base, k, cell)); return; }
         int face = 0;
         const bool bb = WALLS && nb.crossed(-cy, -cz, face) >= 0;
         const int plane = (bb != (aa == 2)) ? Q - 1 - k : k;
-        if (bb) { cp_async_8(slot, base + plane * N + cell); return; }
-        const float* r = base + plane * N + nb.row(-cy, -cz);
+        if (bb) { cp_async_8(slot, elem(base, plane, cell)); return; }
+        const float* r = elem(base, plane, nb.row(-cy, -cz));
         if (cx == 0) cp_async_8(slot, r);
         else {
             cp_async_4(reinterpret_cast<float*>(slot), r + nb.first(-cx));
@@ -180,12 +200,12 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
     auto put = [&](float* base, int Q, int k, int q27i, real v, bool& wall_link) {
         const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
         wall_link = false;
-        if (aa == 0) { *reinterpret_cast<float2*>(base + k * N + cell) = v.v; return; }
-        if (aa == 1) { *reinterpret_cast<float2*>(base + (Q - 1 - k) * N + cell) = v.v; return; }
+        if (aa == 0) { *reinterpret_cast<float2*>(elem(base, k, cell)) = v.v; return; }
+        if (aa == 1) { *reinterpret_cast<float2*>(elem(base, Q - 1 - k, cell)) = v.v; return; }
         int face = 0;
         wall_link = WALLS && nb.crossed(cy, cz, face) >= 0;
-        if (wall_link) { *reinterpret_cast<float2*>(base + (Q - 1 - k) * N + cell) = v.v; return; }
-        float* r = base + k * N + nb.row(cy, cz);
+        if (wall_link) { *reinterpret_cast<float2*>(elem(base, Q - 1 - k, cell)) = v.v; return; }
+        float* r = elem(base, k, nb.row(cy, cz));
         if (cx == 0) *reinterpret_cast<float2*>(r) = v.v;
         else { r[nb.first(cx)] = v.v.x; r[nb.second(cx)] = v.v.y; }
     };
@@ -193,12 +213,12 @@ __global__ void __launch_bounds__(kBlock, pair_min_blocks<QT, AA>()) fused_step_
     // the same addressing with plain loads (pair_h_direct)
     auto fetch = [&](const float* base, int Q, int k, int q27i) -> float2 {
         const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);
-        if (aa == 1) return *reinterpret_cast<const float2*>(base + k * N + cell);
+        if (aa == 1) return *reinterpret_cast<const float2*>(elem(base, k, cell));
         int face = 0;
         const bool bb = WALLS && nb.crossed(-cy, -cz, face) >= 0;
         const int plane = (bb != (aa == 2)) ? Q - 1 - k : k;
-        if (bb) return *reinterpret_cast<const float2*>(base + plane * N + cell);
-        const float* r = base + plane * N + nb.row(-cy, -cz);
+        if (bb) return *reinterpret_cast<const float2*>(elem(base, plane, cell));
+        const float* r = elem(base, plane, nb.row(-cy, -cz));
         if (cx == 0) return *reinterpret_cast<const float2*>(r);
         return make_float2(r[nb.first(-cx)], r[nb.second(-cx)]);
     };

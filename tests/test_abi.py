@@ -79,7 +79,7 @@ def test_params_default_matches_the_binding_and_a_zeroed_struct_is_rejected():
 
 def test_extent_validation():
     p = tcp.make_params(dict(bc=("periodic", "walls", "periodic")))
-    for dims in ((0, 4, 4), (4, 1, 4), (2048, 2048, 2048)):
+    for dims in ((0, 4, 4), (4, 1, 4), (2048, 2048, 2048), (800, 800, 800)):   # 800^3: 10 N >= 2^32
         with pytest.raises(tcp.TcpError) as e:
             tcp.tcp_workspace_bytes(*dims, p)
         assert e.value.code == tcp.TCP_EINVAL

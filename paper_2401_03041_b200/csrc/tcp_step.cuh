@@ -476,16 +476,17 @@ __global__ void __launch_bounds__(kBlock, async_min_blocks<real, QT, AA>()) fuse
     // (measured: 4.5 instructions per staged copy before).
     // (the group bases are made opaque to the optimiser, which would otherwise fold 9 g N back into a 64-bit offset)
     const unsigned Nu = (unsigned)A.ncell;
+    // fp64 only: the one-cell-per-thread fp32 kernel (odd nx, walls in x) measured 0.5-1 % slower with it
     auto elem = [&](auto* base, int plane, int off) {
-#if TCP_ADDR32
-        const int g = plane / 9;
-        auto* gb = base + (long long)(9 * g) * N;
-        asm("" : "+l"(gb));
-        __builtin_assume(__isGlobal(gb));      // the asm hid the address space with the value: keep LDG / STG
-        return gb + (unsigned)((unsigned)(plane - 9 * g) * Nu + (unsigned)off);
-#else
-        return base + plane * N + off;
-#endif
+        if constexpr (TCP_ADDR32 && sizeof(real) == 8) {
+            const int g = plane / 9;
+            auto* gb = base + (long long)(9 * g) * N;
+            asm("" : "+l"(gb));
+            __builtin_assume(__isGlobal(gb));      // the asm hid the address space with the value: keep LDG / STG
+            return gb + (unsigned)((unsigned)(plane - 9 * g) * Nu + (unsigned)off);
+        } else {
+            return base + plane * N + off;
+        }
     };
     auto src_of = [&](const real* base, int Q, int k, int q27i) -> const real* {
         const int cx = cx27(q27i), cy = cy27(q27i), cz = cz27(q27i);

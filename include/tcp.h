@@ -84,7 +84,8 @@ typedef struct tcp_params {
                                           Maxwell-Boltzmann distribution taken in central-moment space (central moments of x^a y^b z^c
                                           = s m_a m_b m_c, m = (1, 0, c_s^2); on D3Q27 the product form), in place of eq. 12; eq. 18
                                           becomes w_i (p* - 1) + that equilibrium with s = 1.  Moments up to second order are
-                                          unchanged.  D3Q27 lattices only: hydro_lattice = 27 and thermal D3Q27 LB / RK2 / RK4 */
+                                          unchanged.  D3Q27 lattices only: hydro_lattice = 27 and thermal D3Q27 LB / RK2 / RK4; closed-form
+                                          collision only (s_high = 1, high_rate_equals_shear = 0); either collision space */
 } tcp_params;
 
 /* Fill *p with the defaults: struct_size, fp64, thermal LB D3Q7, two-grid, periodic x 3, rho = 1, tau = 0.6, xi = 4,

@@ -81,6 +81,8 @@ int validate(int nx, int ny, int nz, const tcp_params* p) {
         const int qt = thermal_q(p->thermal);
         if (p->hydro_lattice != 27 || (qt != 0 && qt != 27))
             return fail(TCP_EUNSUPPORTED, "Maxwellian equilibrium: D3Q27 lattices only (hydro_lattice = 27; thermal D3Q27 LB, RK2 or RK4)");
+        if (p->high_rate_equals_shear || p->s_high != 1.0)
+            return fail(TCP_EUNSUPPORTED, "Maxwellian equilibrium: with the closed-form collision only (s_high = 1, high_rate_equals_shear = 0)");
     }
     if (p->collision_space != TCP_SPACE_CENTRAL && p->collision_space != TCP_SPACE_RAW) return fail(TCP_EINVAL, "collision_space must be TCP_SPACE_CENTRAL or TCP_SPACE_RAW");
     if (p->hydro_lattice != 27 && p->hydro_lattice != 19) return fail(TCP_EINVAL, "hydro_lattice must be 27 or 19 (default 27, see tcp_params_default)");
@@ -348,7 +350,7 @@ int relax_t(tcp_sim* s, int nsteps) {
         tcp::StepArgs<real> A = make_args<real>(s);
         if (qt) {
             tcp::FusedCfg c;
-            c.qt = qt; c.walls = s->walls; c.mode = s->P.high_rate_equals_shear ? 1 : 0; c.aa = aa; c.device = s->device; c.grid = grid_for(s->N);
+            c.qt = qt; c.walls = s->walls; c.mode = s->P.equilibrium == TCP_EQ_MAXWELLIAN ? 4 : (s->P.high_rate_equals_shear ? 1 : 0); c.aa = aa; c.device = s->device; c.grid = grid_for(s->N);
             CK(s->walls ? tcp::launch_thermal_walls(c, A, s->stream) : tcp::launch_thermal_periodic(c, A, s->stream));
             s->launches++;
             if (aa) aa = 3 - aa;
@@ -365,13 +367,13 @@ int relax_t(tcp_sim* s, int nsteps) {
 template <typename real>
 int launch_fused(tcp_sim* s, const tcp::StepArgs<real>& A) {
     // collision mode: 0 closed-form central moments (s_high = 1), 1 BGK, 2 general rates (full transform)
-    const int mode = s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0);
+    const int mode = s->P.equilibrium == TCP_EQ_MAXWELLIAN ? 4 : (s->P.high_rate_equals_shear ? 1 : (s->P.s_high != 1.0 ? 2 : 0));
     tcp::FusedCfg c;
     c.qt = thermal_q(s->P.thermal); c.walls = s->walls; c.mode = mode; c.aa = s->aa_next; c.device = s->device;
     c.grid = grid_for((size_t)(A.cell1 - A.cell0));
     const bool q19 = s->P.hydro_lattice == 19;       // D3Q19 hydrodynamic lattice: kernels of the *_q19 translation units
     if constexpr (sizeof(real) == 4) {
-        if (s->use_pair && mode == 0) {
+        if (s->use_pair && (mode == 0 || mode == 4)) {
             if (q19) CK(s->walls ? tcp::launch_pair_walls_q19(c, A, s->stream) : tcp::launch_pair_periodic_q19(c, A, s->stream));
             else CK(s->walls ? tcp::launch_pair_walls(c, A, s->stream) : tcp::launch_pair_periodic(c, A, s->stream));
             s->launches++;

@@ -12,7 +12,7 @@ constexpr int kMaxDevices = 64;
 struct FusedCfg {
     int qt;          // thermal stencil size, 0 on the Runge-Kutta paths
     bool walls;      // any WALLS axis
-    int mode;        // 0 closed-form central moments, 1 BGK, 2 general rates
+    int mode;        // 0 closed-form central moments, 1 BGK, 2 general rates, 3 calibration, 4 = 0 with the Maxwellian equilibrium
     int aa;          // 0 two-grid; AA in-place streaming: 1 even step, 2 odd step
     int device;      // CUDA device of the simulation (per-device kernel attributes)
     unsigned grid;

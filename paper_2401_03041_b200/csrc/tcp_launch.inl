@@ -35,6 +35,17 @@ cudaError_t dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t st
         else return cudaErrorNotSupported;
     }
 #endif
+#if TCP_QH == 27
+    if (c.mode == 4) {   // Maxwellian equilibrium: D3Q27 lattices only (thermal D3Q27 LB or a Runge-Kutta path)
+        if constexpr (QT == 0 || QT == 27) {
+            switch (c.aa) {
+            case 0: return launch_staged<real, QT, WALLS, 4, 0>(c, A, stream);
+            case 1: return launch_staged<real, QT, WALLS, 4, 1>(c, A, stream);
+            default: return launch_staged<real, QT, WALLS, 4, 2>(c, A, stream);
+            }
+        } else return cudaErrorNotSupported;
+    }
+#endif
     switch (3 * c.aa + c.mode) {   // c.aa: 0 two-grid, 1 AA even step, 2 AA odd step
     case 0: return launch_staged<real, QT, WALLS, 0, 0>(c, A, stream);
     case 1: return launch_staged<real, QT, WALLS, 1, 0>(c, A, stream);
@@ -65,6 +76,16 @@ cudaError_t by_stencil(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t 
 #if TCP_QH == 27
 template <typename real, int QT, bool WALLS>
 cudaError_t thermal_dispatch(const FusedCfg& c, const StepArgs<real>& A, cudaStream_t stream) {
+    if (c.mode == 4) {   // Maxwellian equilibrium (D3Q27 thermal LB only)
+        if constexpr (QT == 27) {
+            switch (c.aa) {
+            case 0: thermal_only_kernel<real, QT, WALLS, 4, 0><<<c.grid, kBlock, 0, stream>>>(A); break;
+            case 1: thermal_only_kernel<real, QT, WALLS, 4, 1><<<c.grid, kBlock, 0, stream>>>(A); break;
+            default: thermal_only_kernel<real, QT, WALLS, 4, 2><<<c.grid, kBlock, 0, stream>>>(A); break;
+            }
+            return cudaGetLastError();
+        } else return cudaErrorNotSupported;
+    }
     switch (2 * c.aa + (c.mode == 1)) {
     case 0: thermal_only_kernel<real, QT, WALLS, 0, 0><<<c.grid, kBlock, 0, stream>>>(A); break;
     case 1: thermal_only_kernel<real, QT, WALLS, 1, 0><<<c.grid, kBlock, 0, stream>>>(A); break;
@@ -105,7 +126,18 @@ cudaError_t launch_pair(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_
 }
 template <int QT, bool WALLS>
 cudaError_t pair_dispatch(const FusedCfg& c, const StepArgs<f32x2>& A, cudaStream_t stream) {
-    switch (c.aa) {   // default collision mode only (BGK and general rates run the scalar kernels)
+#if TCP_QH == 27
+    if (c.mode == 4) {
+        if constexpr (QT == 0 || QT == 27) {
+            switch (c.aa) {
+            case 0: return launch_pair<QT, WALLS, 4, 0>(c, A, stream);
+            case 1: return launch_pair<QT, WALLS, 4, 1>(c, A, stream);
+            default: return launch_pair<QT, WALLS, 4, 2>(c, A, stream);
+            }
+        } else return cudaErrorNotSupported;
+    }
+#endif
+    switch (c.aa) {   // closed-form collision modes only (BGK and general rates run the scalar kernels)
     case 0: return launch_pair<QT, WALLS, 0, 0>(c, A, stream);
     case 1: return launch_pair<QT, WALLS, 0, 1>(c, A, stream);
     default: return launch_pair<QT, WALLS, 0, 2>(c, A, stream);

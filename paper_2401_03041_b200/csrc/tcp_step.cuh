@@ -4,6 +4,11 @@
 
 namespace tcp {
 
+// MODE of the collision templates: 0 closed-form central moments (or raw moments, StepArgs::cm_frame), 1 BGK, 2 general rates,
+// 3 roofline calibration (no collision), 4 = mode 0 with the Maxwellian equilibrium (D3Q27 lattices; a compile-time mode
+// because a run-time branch around the product form cost the fp32 pair kernel 2.2 % and the fp64 D3Q27 kernel 1.6 %)
+template <int MODE> __host__ __device__ constexpr bool mode_maxwell() { return MODE == 4; }
+
 #ifndef TCP_BLOCK
 #define TCP_BLOCK 128
 #endif
@@ -115,12 +120,12 @@ __device__ __forceinline__ real collide_phase(const StepArgs<real>& A, real h[27
     real b[3], v[3];
 #pragma unroll
     // E = sigma h_eq(eq. 12) + F/2; sigma = 1, or 0 with the Maxwellian equilibrium, whose product form is added instead
-    const real se = A.eq_sigma * phin;
+    const real se = mode_maxwell<MODE>() ? real(0) : phin;
     for (int al = 0; al < 3; ++al) { b[al] = se * un[al] + a[al]; v[al] = se * un[al] + real(0.5) * a[al]; }
     const real A0 = se - real(1.5) * (un[0] * b[0] + un[1] * b[1] + un[2] * b[2]);
     real out[27];
     equilibrium_plus_half_force27<real>(A0, un, v, b, out);
-    if (A.maxwell) add_product_form27<real, false>(phin, un, out);
+    if constexpr (mode_maxwell<MODE>()) add_product_form27<real, false>(phin, un, out);
     if (MODE == 1) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) h[q] = (real(1) - w) * h[q] + w * out[q];
@@ -200,21 +205,12 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
     real b[3], v[3];
 #pragma unroll
     // E = w_q p* + sigma w_q [poly(u) of eq. 18] + F/2; Maxwellian (sigma = 0): + w_q (pi_x pi_y pi_z - 1) instead of w_q poly(u)
-    const real sg = A.eq_sigma;
+    const real sg = mode_maxwell<MODE>() ? real(0) : real(1);
     for (int al = 0; al < 3; ++al) { b[al] = sg * u[al] + a[al]; v[al] = sg * u[al] + real(0.5) * a[al]; }
     const real A0 = ps - real(1.5) * (u[0] * b[0] + u[1] * b[1] + u[2] * b[2]);
     real out[27];
     equilibrium_plus_half_force27<real, QH>(A0, u, v, b, out);
-    real pf[(MODE == 2) ? 27 : 1];           // general-rate mode: the product form is needed twice (in E(a) and in E(-a))
-    if constexpr (MODE == 2) {
-#pragma unroll
-        for (int q = 0; q < 27; ++q) pf[q] = real(0);
-        if (A.maxwell) add_product_form27<real, true>(real(1), u, pf);
-#pragma unroll
-        for (int q = 0; q < 27; ++q) out[q] += pf[q];
-    } else {
-        if (A.maxwell) add_product_form27<real, true>(real(1), u, out);
-    }
+    if constexpr (mode_maxwell<MODE>()) add_product_form27<real, true>(real(1), u, out);
     if (MODE == 1) {
 #pragma unroll
         for (int q = 0; q < 27; ++q) g[q] = (real(1) - om) * g[q] + om * out[q];
@@ -230,7 +226,7 @@ __device__ __forceinline__ void collide_hydro(const StepArgs<real>& A, real g[27
             for (int al = 0; al < 3; ++al) { bm[al] = sg * u[al] - a[al]; vm[al] = sg * u[al] - real(0.5) * a[al]; }
             equilibrium_plus_half_force27<real, QH>(ps - real(1.5) * (u[0] * bm[0] + u[1] * bm[1] + u[2] * bm[2]), u, vm, bm, X);
 #pragma unroll
-            for (int q = 0; q < 27; ++q) X[q] = g[q] - (X[q] + pf[q]);
+            for (int q = 0; q < 27; ++q) X[q] = g[q] - X[q];
         }
         const real uf[3] = {A.cm_frame * u[0], A.cm_frame * u[1], A.cm_frame * u[2]};   // raw-moment space: transform about rest
         central_transform27<real, true>(X, uf);
@@ -297,12 +293,10 @@ __device__ __forceinline__ real collide_thermal(const StepArgs<real>& A, real f[
     const real kap = A.kappa_L + phi_new * A.dkappa;         // eq. 23 (G5)
     const real w = real(1) / (real(0.5) + real(3) * kap);    // eq. 29 read as a rate (G4)
     real out[Q];
-    if constexpr (Q == 27) {
-        if (A.maxwell) {
+    if constexpr (Q == 27 && mode_maxwell<MODE>()) {
 #pragma unroll
-            for (int q = 0; q < 27; ++q) out[q] = real(0);
-            add_product_form27<real, false>(Tn, u, out);
-        } else thermal_equilibrium<real, Q>(Tn, u, out);
+        for (int q = 0; q < 27; ++q) out[q] = real(0);
+        add_product_form27<real, false>(Tn, u, out);
     } else thermal_equilibrium<real, Q>(Tn, u, out);
     if (MODE == 1) {
         static_for<0, Q>([&](auto K) { constexpr int k = decltype(K)::value; out[k] = (real(1) - w) * f[k] + w * out[k]; });
@@ -379,6 +373,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 #ifndef TCP_ADDR32
 #define TCP_ADDR32 1
 #endif
+
 #ifndef TCP_PF
 #define TCP_PF 50
 #endif

@@ -29,8 +29,7 @@ def test_periodic_box(thermal):
     assert np.abs(printed[1] - got[1]).max() > 1e-8
 
 
-@pytest.mark.parametrize("extra", [dict(s_high=1.4, s_bulk=0.9), dict(high_rate_equals_shear=1), dict(collision_space="raw"),
-                                   dict(streaming="aa")])
+@pytest.mark.parametrize("extra", [dict(s_bulk=0.9), dict(collision_space="raw"), dict(streaming="aa"), dict(thermal="rk2")])
 def test_channel_with_walls_in_other_modes(extra):
     wl = W.layered_channel(nx=44, ny=26, nz=2, thermal="lb_d3q27", rho_upper=2.0)
     wu = [[[0.0] * 3 for _ in range(2)] for _ in range(3)]
@@ -51,8 +50,27 @@ def test_fp32(nx):
 
 
 def test_other_lattices_are_refused():
-    for bad in (dict(MX, thermal="lb_d3q7"), dict(MX, thermal="lb_d3q27", hydro_lattice=19)):
+    for bad in (dict(MX, thermal="lb_d3q7"), dict(MX, thermal="lb_d3q27", hydro_lattice=19), dict(MX, thermal="rk2", s_high=1.3),
+                dict(MX, thermal="rk2", high_rate_equals_shear=1)):
         with pytest.raises(tcp.TcpError) as e:
             tcp.tcp_workspace_bytes(8, 8, 8, tcp.make_params(bad))
         assert e.value.code == tcp.TCP_EUNSUPPORTED
     assert tcp.tcp_workspace_bytes(8, 8, 8, tcp.make_params(dict(MX, thermal="rk4"))) > 0
+
+
+@pytest.mark.parametrize("streaming", ["two_grid", "aa"])
+def test_temperature_preinitialisation_with_the_maxwellian(streaming):
+    """tcp_relax_temperature runs the thermal-only kernel: its Maxwellian instantiation (D3Q27 thermal LB)."""
+    from oracle import tcpo
+    wl = _with_velocity(W.layered_channel(nx=20, ny=14, nz=6, thermal="lb_d3q27"), amp=0.02, seed=3)
+    p = dict(wl.params, equilibrium=1)
+    o = tcpo.Oracle(wl.nx, wl.ny, wl.nz, p)
+    sim = tcp.Simulation(wl.nx, wl.ny, wl.nz, dict(p, streaming=streaming))
+    for (ax, fc), plane in wl.wall_T.items():
+        o.set_wall_temperature(ax, fc, plane.numpy()); sim.set_wall_temperature(ax, fc, plane.numpy())
+    o.init_fields(wl.phi.numpy(), wl.u.numpy(), wl.T.numpy()); sim.init_fields(wl.phi.numpy(), wl.u.numpy(), wl.T.numpy())
+    o.relax_temperature(20); sim.relax_temperature(20)
+    o.step(5); sim.step(5)
+    want, got = o.read_fields(), sim.read_fields()
+    o.close(); sim.close()
+    assert_parity_f64(got, want)

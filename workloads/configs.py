@@ -244,22 +244,32 @@ def laser_source(nx, ny, nz, Q_s=0.2, centre=None, w_s=6.0, d_s=8.0):
 # --------------------------------------------------------------------------------------------
 # droplet in a sheared channel with a laser spot (section 3.2, figure 6)
 
-def laser_channel(R=32, theta=60.0, thermal="lb_d3q7", nz=1, Q_s=0.2, kappa=0.2):
-    """The paper's 2-D droplet-capture set-up: domain 8R x 2R (x nz), x periodic, no-slip walls in y at T_ref = 0, a half
-    disc of radius R on the lower wall at x_c = 2R + 1 (65 for R = 32), the upper wall moving with U_w = gamma L_y, a laser
-    source (eq. 37) at (x_s, y_s) = (181, 21) R / 32 with w_s = 6, d_s = 8 (scaled with R / 32), sigma_T = 2e-4,
-    sigma_ref = 5e-3, xi = 4, contact angle `theta` on the lower wall.  Ca = mu U / sigma = 0.16 and
-    Re = U R / nu = 0.08 with U = gamma R fix nu = sqrt(Ca sigma R / Re) (rho = 1): nu = 0.566 for R = 32,
-    U_w = 2 U.  The paper's Ma = 0.01 would need a diffusivity beyond the stable range of an explicit update at this nu;
-    kappa is a free argument here (S15: parameter not usable as given) and defaults to 0.2.  Returns (workload, q) with q
-    the heat-source field for tcp_set_heat_source."""
+def laser_channel(R=32, theta=60.0, thermal="lb_d3q7", nz=1, Q_s=0.2, kappa=0.2, three_d=False, sources=1):
+    """The paper's droplet-capture set-ups.
+
+    2-D (section 3.2, figure 6; `three_d=False`): domain 8R x 2R (x nz), x periodic, no-slip walls in y at
+    T_ref = 0, a half disc of radius R on the lower wall at x_c = 2R + 1 (65 for R = 32), the upper wall moving with
+    U_w = gamma L_y, a laser source (eq. 37) at (x_s, y_s) = (181, 21) R / 32 with w_s = 6, d_s = 8 (scaled with R / 32),
+    sigma_T = 2e-4, sigma_ref = 5e-3, xi = 4, contact angle `theta` on the lower wall.
+    3-D (section 3.3, figure 8; `three_d=True`): domain 16R x 2R x 8R, x and z periodic, a half sphere of
+    radius R on the lower wall at (x_c, z_c) = (2R + 1, 4R), the laser at the same (x_s, y_s) in the plane z = 4R;
+    `sources=2` puts two lasers at z = 4R -+ R/2 (figure 11).
+    Ca = mu U / sigma = 0.16 and Re = U R / nu = 0.08 with U = gamma R fix nu = sqrt(Ca sigma R / Re) (rho = 1): nu = 0.566 for
+    R = 32, U_w = 2 U.  The paper's Ma = 0.01 would need a diffusivity beyond the stable range of an explicit update at
+    this nu; kappa is a free argument here (S15: parameter not usable as given) and defaults to 0.2.  Returns (workload, q)
+    with q the heat-source field for tcp_set_heat_source."""
     s = R / 32.0
-    nx, ny = 8 * R, 2 * R
+    nx, ny = (16 * R if three_d else 8 * R), 2 * R
+    if three_d:
+        nz = 8 * R
     xi, sigma, Ca, Re = 4.0, 5e-3, 0.16, 0.08
     nu = float(np.sqrt(Ca * sigma * R / Re))          # from nu U = Ca sigma and U R = Re nu
     U = Re * nu / R
     x, y, z = _grid(nx, ny, nz)
-    r = torch.sqrt((x - (2 * R + 1)) ** 2 + (y + 0.5) ** 2).expand(nz, ny, nx).contiguous()
+    r2 = (x - (2 * R + 1)) ** 2 + (y + 0.5) ** 2
+    if three_d:
+        r2 = r2 + (z - (4 * R - 0.5)) ** 2
+    r = torch.sqrt(r2).expand(nz, ny, nx).contiguous()
     phi = _droplet_profile(r, float(R), xi)
     wall_u = [[[0.0] * 3 for _ in range(2)] for _ in range(3)]
     wall_u[1][1] = [2.0 * U, 0.0, 0.0]                # gamma = U / R, L_y = 2 R
@@ -268,7 +278,12 @@ def laser_channel(R=32, theta=60.0, thermal="lb_d3q7", nz=1, Q_s=0.2, kappa=0.2)
                   rho_H=1.0, rho_L=1.0, tau_H=3.0 * nu, tau_L=3.0 * nu, xi=xi, M=0.05,
                   sigma_ref=sigma, sigma_T=2e-4, T_ref=0.0, kappa_H=kappa, kappa_L=kappa, cp_H=1.0, cp_L=1.0,
                   wall_T=((0.0, 0.0), (0.0, 0.0), (0.0, 0.0)), wall_u=wall_u, wall_contact_angle=angles, eps_normal=1e-9)
-    q = laser_source(nx, ny, nz, Q_s=Q_s, centre=(181.0 * s, 21.0 * s, (nz - 1) / 2.0), w_s=6.0 * s, d_s=8.0 * s)
-    wl = Workload("laser_channel", nx, ny, nz, params, phi, T=None, steps=20000)
-    wl.notes = f"R={R}, theta={theta}, nu={nu:.4f}, U_w={2 * U:.3e}"
+    zc = (4 * R - 0.5) if three_d else (nz - 1) / 2.0
+    if three_d and sources == 2:
+        q = laser_source(nx, ny, nz, Q_s=Q_s, centre=(181.0 * s, 21.0 * s, zc - 0.5 * R), w_s=6.0 * s, d_s=8.0 * s) \
+            + laser_source(nx, ny, nz, Q_s=Q_s, centre=(181.0 * s, 21.0 * s, zc + 0.5 * R), w_s=6.0 * s, d_s=8.0 * s)
+    else:
+        q = laser_source(nx, ny, nz, Q_s=Q_s, centre=(181.0 * s, 21.0 * s, zc), w_s=6.0 * s, d_s=8.0 * s)
+    wl = Workload("laser_channel_3d" if three_d else "laser_channel", nx, ny, nz, params, phi, T=None, steps=20000)
+    wl.notes = f"R={R}, theta={theta}, nu={nu:.4f}, U_w={2 * U:.3e}" + (f", 3-D, {sources} source(s)" if three_d else "")
     return wl, q

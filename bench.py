@@ -286,26 +286,25 @@ def run_ours(args):
     if not args.no_e2e:
         hp = torch.empty((n, n, n), dtype=tdt, pin_memory=True); hp.copy_(phi_d)
         hT = torch.empty((n, n, n), dtype=tdt, pin_memory=True); hT.copy_(T_d)
-        hu = torch.zeros((3, n, n, n), dtype=tdt, pin_memory=True)
         o_phi = torch.empty((n, n, n), dtype=tdt, pin_memory=True); o_T = torch.empty_like(o_phi); o_p = torch.empty_like(o_phi)
         o_u = torch.empty((3, n, n, n), dtype=tdt, pin_memory=True)
         for t in (o_phi, o_T, o_p, o_u):   # touch the pages: the first DMA into fresh pinned memory runs at ~6 GB/s
             t.zero_()
         barrier()
         t0 = time.perf_counter()
-        tcp.tcp_init_fields(sim._h, hp, hu, hT)            # H2D of phi, u, T + equilibrium init
+        tcp.tcp_init_fields(sim._h, hp, None, hT)          # H2D of phi and T (the workload starts at rest: u = NULL) + equilibrium init
         tcp.tcp_step(sim._h, args.steps)
         tcp.tcp_read_fields(sim._h, o_phi, o_u, o_p, o_T)  # pressure kernel + D2H of phi, u, p, T (synchronises)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         dt_max = max_over_ranks(dt * 1e3, dist)
         e2e = {"value": aggregate_mlups(N, args.steps, world, dt_max), "unit": "MLUPS",
-               "h2d_bytes_per_step": 5 * N * es / args.steps, "d2h_bytes_per_step": 6 * N * es / args.steps,
-               "steps": args.steps, "h2d_bytes": 5 * N * es, "d2h_bytes": 6 * N * es, "wall_s": dt_max * 1e-3,
+               "h2d_bytes_per_step": 2 * N * es / args.steps, "d2h_bytes_per_step": 6 * N * es / args.steps,
+               "steps": args.steps, "h2d_bytes": 2 * N * es, "d2h_bytes": 6 * N * es, "wall_s": dt_max * 1e-3,
                "note": f"tcp_init_fields(host) + tcp_step({args.steps}) + tcp_read_fields(host), pinned host buffers; the one-off "
                        f"copies of the initial and final fields are amortised over the {args.steps} steps of the call, so this "
                        "figure depends on the step count (state it when quoting)"}
-        del hp, hT, hu, o_phi, o_T, o_p, o_u
+        del hp, hT, o_phi, o_T, o_p, o_u
     sim.close()
     del sim, phi_d, T_d, wl_fields
     torch.cuda.empty_cache()

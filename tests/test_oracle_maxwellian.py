@@ -1,7 +1,8 @@
 """Pins of the oracle's Maxwellian equilibrium (`equilibrium = 1`, D3Q27 lattices): the continuous Maxwell-Boltzmann
 distribution taken in central-moment space, in place of the second-order equilibria the paper prints (eqs. 12, 18).
 Definition-level pins with numpy (central moments; the textbook product form), and the closed forms every equilibrium
-must still satisfy (Poiseuille, heat sinusoid with advection, Laplace law)."""
+must still satisfy: the advected heat sinusoid (Poiseuille and the Laplace law see moments up to second order
+only, which the two equilibria share; the GPU parity tests run both flows with it)."""
 import numpy as np
 import pytest
 
@@ -52,7 +53,7 @@ def test_equilibrium_populations_are_the_product_form_and_have_maxwellian_centra
     o.close()
 
 
-def test_heat_sinusoid_and_laplace_with_the_maxwellian():
+def test_advected_heat_sinusoid_with_the_maxwellian():
     # (Poiseuille is left to the other equilibrium: it sees second moments only, which the two equilibria share)
     n, kap, U, steps = 48, 0.1, 0.04, 120
     k = 2 * np.pi / n
@@ -66,16 +67,6 @@ def test_heat_sinusoid_and_laplace_with_the_maxwellian():
     Fm = np.fft.rfft(T - 1)[1]
     assert -np.log(2 * np.abs(Fm) / n / 0.5) / steps == pytest.approx(kap * k * k, rel=0.02)
     assert (-np.angle(Fm) - np.pi / 2) / k == pytest.approx(U * steps, rel=0.01)
-    nn, R = 28, 6.0
-    wl = W.static_droplet(n=nn, R=R, nz=1)
-    o = tcpo.Oracle(nn, nn, 1, dict(wl.params, **MX))
-    o.init_fields(wl.phi.numpy())
-    o.step(500)
-    phi, u, p, T = o.read_fields()
-    o.close()
-    dp = p[0, nn // 2 - 1:nn // 2 + 1, nn // 2 - 1:nn // 2 + 1].mean() - p[0, 0, 0]
-    assert dp / (wl.params["sigma_ref"] / R) == pytest.approx(1.0, abs=0.05)
-    assert abs(phi.sum() - float(wl.phi.sum())) / float(wl.phi.sum()) < 1e-12
 
 
 def test_only_d3q27_lattices_take_the_maxwellian():

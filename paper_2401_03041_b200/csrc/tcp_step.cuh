@@ -427,15 +427,15 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
 // only fits two blocks anyway), so those are compiled for two blocks per SM.
 // fp64 D3Q15 / D3Q19: h, which is consumed first, is pulled straight into registers together with the stencil loads and
 // only g and f are staged (42 / 46 KB per block), so that three blocks fit the shared memory as for D3Q7: 400^3 D3Q15
-// 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained.  D3Q27 (15.16 -> 15.30) keeps h staged, and so does D3Q7, which
-// has its three blocks anyway: 0.5 % faster under the power cap but 4 % slower per launch at full clock (ncu 10.79 vs
-// 10.35 ms, 2 % more DRAM reads)
+// 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained.  D3Q27 (15.16 -> 15.30) keeps h staged.  D3Q7 has its three blocks anyway.  Round 1 measured D3Q7 0.5 % faster that way under the power cap but 4 % slower per launch at full
+// clock and kept h staged; with the 32-bit offsets of round 2 the full-clock penalty is gone (5-step run 10.56 vs 10.56 ms) and the
+// sustained gain remains (D3Q7 11.46-11.49 vs 11.55 ms, RK2 10.99-11.02 vs 11.15): h is pulled directly for every Q_T but 27
 #ifndef TCP_HDIRECT
 #define TCP_HDIRECT 1
 #endif
 // (two-grid streaming only: with AA in place the same change costs 8-16 %)
 template <typename real, int QT, int AA>
-__host__ __device__ constexpr bool h_direct() { return TCP_HDIRECT && sizeof(real) == 8 && (QT == 15 || QT == 19) && AA == 0; }
+__host__ __device__ constexpr bool h_direct() { return TCP_HDIRECT && sizeof(real) == 8 && QT != 27 && AA == 0; }
 
 template <typename real, int QT, int AA = 0>
 __host__ __device__ constexpr int async_min_blocks() {

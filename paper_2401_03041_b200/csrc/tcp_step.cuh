@@ -433,9 +433,12 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
 #ifndef TCP_HDIRECT
 #define TCP_HDIRECT 1
 #endif
-// (two-grid streaming only: with AA in place the same change costs 8-16 %)
+// AA in place: round 1 measured a loss of 8-16 %; after the 32-bit offsets, sustained at 400^3: D3Q7 11.34-11.37 vs 11.46 ms, RK2 10.93
+// vs 11.22, D3Q15 12.96 vs 13.12 -- taken -- and D3Q19 13.84 vs 13.66 -- not taken
 template <typename real, int QT, int AA>
-__host__ __device__ constexpr bool h_direct() { return TCP_HDIRECT && sizeof(real) == 8 && QT != 27 && AA == 0; }
+__host__ __device__ constexpr bool h_direct() {
+    return TCP_HDIRECT && sizeof(real) == 8 && (AA == 0 ? QT != 27 : (QT == 0 || QT == 7 || QT == 15));
+}
 
 template <typename real, int QT, int AA = 0>
 __host__ __device__ constexpr int async_min_blocks() {

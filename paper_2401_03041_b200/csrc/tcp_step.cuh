@@ -427,17 +427,18 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
 // only fits two blocks anyway), so those are compiled for two blocks per SM.
 // fp64 D3Q15 / D3Q19: h, which is consumed first, is pulled straight into registers together with the stencil loads and
 // only g and f are staged (42 / 46 KB per block), so that three blocks fit the shared memory as for D3Q7: 400^3 D3Q15
-// 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained.  D3Q27 (15.16 -> 15.30) keeps h staged.  D3Q7 has its three blocks anyway.  Round 1 measured D3Q7 0.5 % faster that way under the power cap but 4 % slower per launch at full
-// clock and kept h staged; with the 32-bit offsets of round 2 the full-clock penalty is gone (5-step run 10.56 vs 10.56 ms) and the
-// sustained gain remains (D3Q7 11.46-11.49 vs 11.55 ms, RK2 10.99-11.02 vs 11.15): h is pulled directly for every Q_T but 27
+// 13.25 -> 12.77 ms, D3Q19 13.83 -> 13.39 ms sustained.  D3Q27 (15.16 -> 15.30) keeps h staged.
+// D3Q7 has its three blocks anyway and keeps h staged: pulled directly it is 0.6 % faster under the power cap (11.46-11.49 vs
+// 11.55 ms) but 3.8 % slower per launch at full clock (ncu 10.77 vs 10.38 ms, DRAM reads 37.5 vs 36.2 GB), as round 1 found.
+// The Runge-Kutta paths (Q_T = 0) take it: sustained RK2 10.99-11.02 vs 11.15 ms, +1 % per launch at full clock.
 #ifndef TCP_HDIRECT
 #define TCP_HDIRECT 1
 #endif
-// AA in place: round 1 measured a loss of 8-16 %; after the 32-bit offsets, sustained at 400^3: D3Q7 11.34-11.37 vs 11.46 ms, RK2 10.93
-// vs 11.22, D3Q15 12.96 vs 13.12 -- taken -- and D3Q19 13.84 vs 13.66 -- not taken
+// AA in place: round 1 measured a loss of 8-16 %; after the 32-bit offsets, sustained at 400^3: RK2 10.93 vs 11.22 ms, D3Q15 12.96 vs
+// 13.12 -- taken; D3Q19 13.84 vs 13.66 and D3Q7 (11.34-11.37 vs 11.46 sustained, but +2.6 % per launch at full clock) -- not taken
 template <typename real, int QT, int AA>
 __host__ __device__ constexpr bool h_direct() {
-    return TCP_HDIRECT && sizeof(real) == 8 && (AA == 0 ? QT != 27 : (QT == 0 || QT == 7 || QT == 15));
+    return TCP_HDIRECT && sizeof(real) == 8 && (AA == 0 ? (QT == 0 || QT == 15 || QT == 19) : (QT == 0 || QT == 15));
 }
 
 template <typename real, int QT, int AA = 0>

@@ -19,7 +19,7 @@ import workloads as W
 from oracle import tcpo
 
 
-def _staggered_v(level, steps_a=500, steps_b=1500):
+def _staggered_v(level, steps_a=400, steps_b=1000):
     nx, ny = 64, 32
     wl = W.layered_channel(nx=nx, ny=ny, nz=1)
     o = tcpo.Oracle(nx, ny, 1, dict(wl.params, hydro_phi_level=level))
@@ -42,12 +42,12 @@ def test_s16_phi_n_damps_the_staggered_mode_and_phi_n_plus_1_pumps_it():
     a1, b1, umax1 = _staggered_v(1)
     # the physical flow is the same in both (closed-form interface velocity 2.1e-4 at this resolution) ...
     assert umax0 == pytest.approx(umax1, rel=1e-2) and 1.5e-4 < umax0 < 3e-4
-    # ... but the checkerboard decays with phi^n (measured x0.55 over these 1000 steps, x0.12 over 3500)
-    assert b0 < 0.65 * a0
-    # and grows with phi^{n+1}: measured x1.83 over 1000 steps, doubling time ~1150 steps ("doubles about every 1000")
+    # ... but the checkerboard decays with phi^n (measured x0.55 per 1000 steps, x0.12 over 3500)
+    assert b0 < 0.8 * a0
+    # and grows with phi^{n+1}: measured x1.83 per 1000 steps, doubling time ~1150 steps ("doubles about every 1000")
     growth = b1 / a1
-    assert growth > 1.6
-    doubling = 1000 * np.log(2) / np.log(growth)
+    assert growth > 1.3
+    doubling = 600 * np.log(2) / np.log(growth)
     assert 800 < doubling < 1500
 
 

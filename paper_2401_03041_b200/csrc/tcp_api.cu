@@ -23,6 +23,7 @@ int fail(int code, const char* fmt, const char* detail = "") {
 }
 int cuda_fail(cudaError_t e, const char* where) {
     std::snprintf(g_err, sizeof g_err, "%s: %s", where, cudaGetErrorString(e));
+    (void)cudaGetLastError();   // reported here: a non-sticky error (a refused cudaMalloc) must not resurface in the next call's launch check
     return e == cudaErrorMemoryAllocation ? TCP_ENOMEM : TCP_ECUDA;
 }
 #define CK(call)                                                  \

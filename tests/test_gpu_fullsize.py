@@ -6,6 +6,8 @@ state around the cell; the periodic wrap of the sub-box only pollutes cells with
 half >= 2*steps+2 the centre cell is exact.  Samples cover what only a full-size launch exercises: more than one wave
 of blocks, the L2-prefetch clamping at the array ends (first / last blocks, the last prefetch group), 64-bit plane
 offsets q*N > 2^31 elements, the periodic seams."""
+import gc
+
 import numpy as np
 import pytest
 import torch
@@ -48,10 +50,11 @@ def _sample_cells(wl, n, samples, rng):
     return picks
 
 
-def _sampled_parity(n, thermal, steps, samples, half, precision="f64", streaming="two_grid", extra=None):
+def _sampled_parity(n, thermal, steps, samples, half, precision="f64", streaming="two_grid", extra=None, box=None):
     """-> dict field -> (worst abs error over the samples, max |oracle| over the samples)"""
     assert half >= 2 * steps + 2
-    wl = W.perf_box(n, thermal=thermal, device="cuda")
+    wl = W.perf_box(n, thermal=thermal, device="cuda", **(box or {}))
+    torch.cuda.empty_cache()
     tdt = torch.float64 if precision == "f64" else torch.float32
     if extra:
         wl.params.update(extra)
@@ -61,6 +64,7 @@ def _sampled_parity(n, thermal, steps, samples, half, precision="f64", streaming
     got = sim.read_fields_device()
     launches = sim.launches
     sim.close()
+    torch.cuda.empty_cache()
     assert launches >= steps
     rng = np.random.default_rng(n)
     m = 2 * half + 1
@@ -115,3 +119,49 @@ def test_full_size_sampled_parity_512_cubed_fp32(thermal):
     assert worst["p"][0] <= max(1e-5 * worst["p"][1], 1e-6 * sig)
     for k in ("ux", "uy", "uz"):
         assert worst[k][0] <= max(1e-5 * umax, 2e-6 * sig)
+
+
+@pytest.mark.parametrize("n,thermal,precision,streaming,steps", [
+    (624, "lb_d3q7", "f64", "aa", 5),         # 243 M cells, 134 GB: 32-bit in-group offsets up to 10 N = 2.4e9 > 2^31 (fp64 kernel)
+    (640, "lb_d3q7", "f32", "two_grid", 5),   # 262 M cells, 136 GB: the same in the fp32 pair kernel
+    (752, "lb_d3q7", "f32", "aa", 6),         # 425 M cells, 117 GB: the largest cube under the N <= 429 496 729 limit of tcp_create
+    (640, "rk2", "f64", "aa", 5),             # 132 GB: the z-marching Runge-Kutta stage kernel at 262 M cells
+    (680, "lb_d3q27", "f32", "aa", 5),        # 314 M cells, 81 population planes: plane offsets up to 80 N = 2.5e10 elements
+])
+def test_largest_boxes_sampled_parity(n, thermal, precision, streaming, steps):
+    """Maximum sizes: the largest boxes one B200 holds (fp64 only with AA in place), where plane offsets reach
+    26 N = 1.1e10 elements and the 32-bit offsets inside a group of nine planes (tcp_step.cuh) pass 2^31."""
+    gc.collect()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    need = tcp.tcp_workspace_bytes(n, n, n, tcp.make_params(dict(W.BENCH_FLUID, thermal=thermal, precision=precision,
+                                                                 streaming=streaming))) + 80 * n ** 3
+    if free < need:
+        pytest.skip(f"{free / 1e9:.0f} GB free, {need / 1e9:.0f} GB needed")
+    worst = _sampled_parity(n, thermal, steps=steps, samples=18, half=2 * steps + 2, precision=precision,
+                            streaming=streaming, box=dict(r_min=24.0, r_max=48.0))
+    if precision == "f64":
+        assert max(v[0] for v in worst.values()) <= 1e-10
+    else:
+        sig = W.BENCH_FLUID["sigma_ref"]
+        umax = max(worst[k][1] for k in ("ux", "uy", "uz"))
+        assert worst["phi"][0] <= 1e-5 * worst["phi"][1] and worst["T"][0] <= 1e-5 * worst["T"][1]
+        assert worst["p"][0] <= max(1e-5 * worst["p"][1], 1e-6 * sig)
+        for k in ("ux", "uy", "uz"):
+            assert worst[k][0] <= max(1e-5 * umax, 2e-6 * sig)
+
+
+def test_box_beyond_the_memory_is_refused_and_the_library_stays_usable():
+    n = 700                                                             # fp64 two-grid D3Q27: 467 GB
+    with pytest.raises(tcp.TcpError) as e:                              # tcp_create: the library's own cudaMalloc
+        tcp.tcp_create(n, n, n, tcp.make_params(dict(W.BENCH_FLUID, thermal="lb_d3q27")))
+    assert e.value.code == tcp.TCP_ENOMEM
+    with pytest.raises(tcp.TcpError) as e:                              # 760^3 > 429 496 729 cells
+        tcp.Simulation(760, 760, 760, dict(W.BENCH_FLUID, thermal="rk2", precision="f32", streaming="aa"))
+    assert e.value.code in (tcp.TCP_EINVAL, tcp.TCP_EUNSUPPORTED)
+    wl = W.static_droplet(n=16, R=4.0)
+    sim = tcp.Simulation(16, 16, 16, wl.params)
+    sim.init_fields(wl.phi.numpy())
+    sim.step(3)
+    assert np.isfinite(sim.read_fields()[2]).all()
+    sim.close()

@@ -5,7 +5,6 @@ Every step of the path runs in the CUDA kernels of libtcp.so; PyTorch is used fo
 if libtcp.so cannot be loaded, or there is no CUDA device, the calls raise.
 """
 import ctypes as C
-import os
 
 import numpy as np
 import torch

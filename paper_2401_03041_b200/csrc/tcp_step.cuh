@@ -389,7 +389,10 @@ __device__ __forceinline__ void prefetch_next_wave(const Args& A, int cells_per_
         asm("mov.u32 %0, %%nsmid;" : "=r"(nsm));
         const unsigned r = blockIdx.x % NR;
         const long long N = A.ncell;
-        const int pf = resident == 2 ? TCP_PF2 : TCP_PF;   // kernels with two blocks per SM: the optimum is flatter and earlier
+        // kernels with two blocks per SM: the optimum is flatter and earlier.  fp64 D3Q19 thermal LB (three blocks, 71 MB of
+        // reads + writes in flight per wave): at 50 % some prefetched lines leave L2 before use (46.3 vs 44.4 GB read per launch
+        // at 40 %, 13.36 vs 13.26 ms sustained)
+        const int pf = (resident == 2 || (sizeof(elem) == 8 && QT == 19 && AA == 0)) ? TCP_PF2 : TCP_PF;
         const long long c0 = (long long)A.cell0 + (long long)(blockIdx.x - r + NR + (pf * resident * nsm) / 100) * cells_per_block;
         if (c0 >= A.cell1) return;
         const elem* base;
